@@ -1,0 +1,140 @@
+/*
+ * fengine.h -- C ABI of the B200-native F-engine (channelizer) data path.
+ *
+ * The path is the one stated in arxiv 2303.09886 Sec. 2.1:
+ *   1. unpack 10-bit signed samples
+ *   2. integer coarse delay as an index offset
+ *   3. T-tap polyphase FIR, Eq. (1)
+ *        g[t] = sum_{j<T} s[N*m - c + t + N*j] * w[t][j],  N = 2n
+ *   4. N-point real-to-complex FFT, keep the n non-negative channels, drop Nyquist
+ *   5. fine delay: X[k] * exp(i(-2 pi d k / N + phi))
+ *   6. complex per-channel gain
+ *   7. quantise to 8-bit signed Gaussian integers, both polarisations interleaved
+ *      (PAPER.md:43, :45, :161): round-half-even, clamp to [-127, 127].
+ * Call names and argument lists follow BASELINE.json:north_star; everything else is this build's
+ * choice (DESIGN.md section 2 lists the readings R1..R18).
+ *
+ * Conventions
+ *   - plain C, no torch types; "host" / "device" is stated for every pointer.
+ *   - every function returning int returns a FENGINE_* status; nothing is thrown across the ABI.
+ *   - a handle is not thread-safe; independent handles are independent.
+ *   - setters copy their host arrays before returning (caller keeps ownership) and take effect
+ *     for later fengine_process calls.  They synchronise the device (off the hot path).
+ *   - there is no CPU fallback: without a CUDA device every call fails with FENGINE_ERR_CUDA.
+ */
+#ifndef FENGINE_H
+#define FENGINE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fengine fengine_t;   /* opaque; one per engine (group of antennas sharing weights) */
+
+enum {
+    FENGINE_OK = 0,
+    FENGINE_ERR_INVALID_ARG = 1,    /* bad size / null pointer / non-finite parameter */
+    FENGINE_ERR_ALLOC = 2,          /* host or device allocation failed */
+    FENGINE_ERR_CUDA = 3,           /* a CUDA call failed (see fengine_last_error) */
+    FENGINE_ERR_STATE = 4           /* tables too short for the requested n_spectra */
+};
+
+/*
+ * fengine_create -- one antenna (an F-engine is the pipeline for the two
+ * polarisations of one antenna).  Same as fengine_create_batched(1, ...).
+ *
+ * n_channels  n, a power of two, 8 <= n <= 32768 (1024, 4096, 8192, 32768).
+ * taps        T, 1 <= T <= 32 (PAPER.md:39: up to 16; :245 measures 32).
+ * n_pols      1 or 2.
+ * weights     HOST, N*T floats, N = 2n, flat time order weights[t + N*j] = w[t][j] of Eq. (1)
+ *             (BASELINE.json configs[0]).  Must be finite.  Copied.
+ * Returns NULL on failure (invalid argument, no device, allocation failure).
+ * Defaults after create: coarse delay 0, fine delay 0, phase 0, gain 1.
+ */
+fengine_t *fengine_create(int n_channels, int taps, int n_pols, const float *weights);
+
+/* n_antennas >= 1 antennas sharing the weights; antenna is the outermost index of in / out. */
+fengine_t *fengine_create_batched(int n_antennas, int n_channels, int taps, int n_pols,
+                                  const float *weights);
+
+void fengine_destroy(fengine_t *fe);
+
+/*
+ * Coarse delays (Eq. (1) index t0 + t - c + 2nj): c in samples, may be negative
+ * or larger than N.  Positive c reads earlier samples.
+ * c             HOST int32 [A][P][n_per_stream].
+ * n_per_stream  1 = one value per stream for the whole call; otherwise entry m applies to spectrum
+ *               m of a fengine_process call and n_per_stream must be >= that call's n_spectra.
+ * Samples whose index falls outside [0, L) read as 0 (R3).
+ */
+int fengine_set_coarse_delays(fengine_t *fe, const int32_t *c, int64_t n_per_stream);
+
+/*
+ * Fine delays: channel k is multiplied by exp(i(-2 pi delay k / N + phase)),
+ * delay in samples, phase in radians (BASELINE.json configs[0]).
+ * delay, phase  HOST float [A][P][n_per_stream], same n_per_stream rule as above.  Must be finite.
+ */
+int fengine_set_fine_delays(fengine_t *fe, const float *delay, const float *phase,
+                            int64_t n_per_stream);
+
+/*
+ * Bandpass gains.
+ * gains_re_im   HOST float [A][P][n][2] (re, im).  Must be finite.
+ */
+int fengine_set_gains(fengine_t *fe, const float *gains_re_im);
+
+/*
+ * fengine_process -- the hot path, steps 1-7 for n_spectra spectra of every stream.
+ *
+ * in         DEVICE, 16-byte aligned, [A][P][L*5/4] bytes, L = N*(n_spectra + T - 1) samples per
+ *            stream: 10-bit two's complement, big-endian bit stream (sample u in bits
+ *            [10u, 10u+10), MSB first, BASELINE.json configs[0]).
+ * out        DEVICE, 16-byte aligned, [A][n_spectra][n][P][2] int8 (re, im).
+ * n_spectra  S >= 0 (0 is a no-op).
+ * stream     a cudaStream_t (NULL = default stream).
+ * Enqueues kernels on `stream` and returns without synchronising; never touches host memory and
+ * never allocates (scratch is sized at create / first call with a larger S -- see DESIGN.md).
+ * Spectrum m of stream (a, p) starts at sample N*m - c[a][p][m] (R2).
+ */
+int fengine_process(fengine_t *fe, const void *in, void *out, int64_t n_spectra, void *stream);
+
+/*
+ * fengine_process_host -- the same path for HOST buffers (the paper's regime: input chunks arrive
+ * in pinned host memory and results go back to the host).
+ * in_host / out_host  HOST pointers (pinned or pageable), same layouts as fengine_process.
+ * Copies the input to device staging owned by the handle (grown on first use), runs the path on an
+ * internal stream, copies the result back and synchronises before returning.
+ */
+int fengine_process_host(fengine_t *fe, const void *in_host, void *out_host, int64_t n_spectra);
+
+/* Human-readable description of the last error on this handle ("" if none). */
+const char *fengine_last_error(const fengine_t *fe);
+
+/* ---- test hooks: same kernels, intermediate results exposed (tolerances are stated on them) ---- */
+
+/* Pre-quantisation spectra Y (after rotation and gain): DEVICE float [A][n_spectra][n][P][2]. */
+int fengine_process_f32(fengine_t *fe, const void *in, float *spectra_out, int64_t n_spectra,
+                        void *stream);
+
+/* Unpacked, coarse-delayed window samples: DEVICE int16 [A][P][n_spectra][N*T] (small cases only):
+ * element i of spectrum m is s[N*m - c + i] (0 outside the batch).  Bit-exact check of steps 1-2. */
+int fengine_debug_unpack(fengine_t *fe, const void *in, int16_t *samples_out, int64_t n_spectra,
+                         void *stream);
+
+/* FIR output g of Eq. (1) in natural column order: DEVICE float [A][P][n_spectra][N]. */
+int fengine_debug_fir(fengine_t *fe, const void *in, float *g_out, int64_t n_spectra, void *stream);
+
+/* Tuning knobs (optional; defaults are chosen at create).  key: "chunk_spectra" (spectra per
+ * L2-resident chunk; 0 = whole call), "fir_rows" (spectra per FIR tile).  Returns INVALID_ARG for
+ * unknown keys. */
+int fengine_set_option(fengine_t *fe, const char *key, int64_t value);
+
+/* Number of kernel launches the last fengine_process / _f32 call enqueued (for bench accounting). */
+int64_t fengine_last_launch_count(const fengine_t *fe);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FENGINE_H */

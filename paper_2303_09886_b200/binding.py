@@ -1,0 +1,171 @@
+"""ctypes binding with the same names as include/fengine.h (argument marshalling only)."""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+
+_PKG = Path(__file__).resolve().parent
+_LIB_PATH = _PKG / "libfengine_b200.so"
+_lib = None
+
+# every symbol include/fengine.h declares (checked by tests/test_abi.py against the header text)
+EXPORTED_SYMBOLS = [
+    "fengine_create", "fengine_create_batched", "fengine_destroy", "fengine_set_coarse_delays",
+    "fengine_set_fine_delays", "fengine_set_gains", "fengine_process", "fengine_process_host",
+    "fengine_last_error", "fengine_process_f32", "fengine_debug_unpack", "fengine_debug_fir",
+    "fengine_set_option", "fengine_last_launch_count",
+]
+
+STATUS = {0: "OK", 1: "INVALID_ARG", 2: "ALLOC", 3: "CUDA", 4: "STATE"}
+
+
+class FEngineError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"fengine error {code} ({STATUS.get(code, '?')}): {msg}")
+        self.code = code
+
+
+def library_path() -> Path:
+    return _LIB_PATH
+
+
+def lib() -> C.CDLL:
+    """Load the CUDA library; fails loudly if it has not been built (no fallback of any kind)."""
+    global _lib
+    if _lib is None:
+        if not _LIB_PATH.exists():
+            raise FileNotFoundError(
+                f"{_LIB_PATH} is missing: build it with `python -m paper_2303_09886_b200.build` "
+                "(there is no CPU fallback)")
+        L = C.CDLL(str(_LIB_PATH))
+        vp, i64 = C.c_void_p, C.c_int64
+        L.fengine_create.argtypes = [C.c_int, C.c_int, C.c_int, vp]
+        L.fengine_create.restype = vp
+        L.fengine_create_batched.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, vp]
+        L.fengine_create_batched.restype = vp
+        L.fengine_destroy.argtypes = [vp]
+        L.fengine_destroy.restype = None
+        L.fengine_set_coarse_delays.argtypes = [vp, vp, i64]
+        L.fengine_set_fine_delays.argtypes = [vp, vp, vp, i64]
+        L.fengine_set_gains.argtypes = [vp, vp]
+        L.fengine_process.argtypes = [vp, vp, vp, i64, vp]
+        L.fengine_process_host.argtypes = [vp, vp, vp, i64]
+        L.fengine_process_f32.argtypes = [vp, vp, vp, i64, vp]
+        L.fengine_debug_unpack.argtypes = [vp, vp, vp, i64, vp]
+        L.fengine_debug_fir.argtypes = [vp, vp, vp, i64, vp]
+        L.fengine_last_error.argtypes = [vp]
+        L.fengine_last_error.restype = C.c_char_p
+        L.fengine_set_option.argtypes = [vp, C.c_char_p, i64]
+        L.fengine_last_launch_count.argtypes = [vp]
+        L.fengine_last_launch_count.restype = i64
+        _lib = L
+    return _lib
+
+
+def _host_ptr(a: np.ndarray):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _dev_ptr(t) -> int:
+    """Device pointer of a torch CUDA tensor (or a raw int)."""
+    if isinstance(t, int):
+        return t
+    if not t.is_cuda or not t.is_contiguous():
+        raise ValueError("expected a contiguous CUDA tensor")
+    return t.data_ptr()
+
+
+def _stream_handle(stream) -> int:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+class FEngine:
+    """One engine: A antennas x P pols sharing the PFB weights (fengine_create_batched)."""
+
+    def __init__(self, n_channels: int, taps: int, n_pols: int, weights, n_antennas: int = 1):
+        w = np.ascontiguousarray(weights, dtype=np.float32).reshape(-1)
+        if w.size != 2 * n_channels * taps:
+            raise ValueError("weights must hold 2*n_channels*taps floats")
+        self._lib = lib()
+        self.A, self.n, self.T, self.P = n_antennas, n_channels, taps, n_pols
+        self.N = 2 * n_channels
+        self._h = self._lib.fengine_create_batched(n_antennas, n_channels, taps, n_pols, _host_ptr(w))
+        if not self._h:
+            raise FEngineError(3, "fengine_create_batched failed (invalid arguments, no CUDA device, or allocation)")
+
+    # -- lifetime -----------------------------------------------------------------------------
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.fengine_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc: int):
+        if rc != 0:
+            raise FEngineError(rc, self._lib.fengine_last_error(self._h).decode())
+
+    # -- setters (host arrays) ------------------------------------------------------------------
+    def set_coarse_delays(self, c):
+        c = np.ascontiguousarray(c, dtype=np.int32).reshape(self.A, self.P, -1)
+        self._check(self._lib.fengine_set_coarse_delays(self._h, _host_ptr(c), c.shape[2]))
+
+    def set_fine_delays(self, delay, phase):
+        d = np.ascontiguousarray(delay, dtype=np.float32).reshape(self.A, self.P, -1)
+        p = np.ascontiguousarray(phase, dtype=np.float32).reshape(self.A, self.P, -1)
+        if d.shape != p.shape:
+            raise ValueError("delay and phase must have the same shape")
+        self._check(self._lib.fengine_set_fine_delays(self._h, _host_ptr(d), _host_ptr(p), d.shape[2]))
+
+    def set_gains(self, gains):
+        g = np.ascontiguousarray(np.asarray(gains, dtype=np.complex64).reshape(self.A, self.P, self.n))
+        self._check(self._lib.fengine_set_gains(self._h, _host_ptr(g.view(np.float32))))
+
+    def set_option(self, key: str, value: int):
+        self._check(self._lib.fengine_set_option(self._h, key.encode(), int(value)))
+
+    # -- sizes ----------------------------------------------------------------------------------
+    def input_bytes(self, n_spectra: int) -> int:
+        return self.A * self.P * (self.N * (n_spectra + self.T - 1) // 4 * 5)
+
+    def output_shape(self, n_spectra: int):
+        return (self.A, n_spectra, self.n, self.P, 2)
+
+    # -- the hot path -----------------------------------------------------------------------------
+    def process(self, inp, out, n_spectra: int, stream=None):
+        """fengine_process: device tensors (uint8 in, int8 out); asynchronous on `stream`."""
+        self._check(self._lib.fengine_process(self._h, _dev_ptr(inp), _dev_ptr(out), n_spectra, _stream_handle(stream)))
+
+    def process_f32(self, inp, out_f32, n_spectra: int, stream=None):
+        self._check(self._lib.fengine_process_f32(self._h, _dev_ptr(inp), _dev_ptr(out_f32), n_spectra,
+                                                  _stream_handle(stream)))
+
+    def process_host(self, inp_host, out_host, n_spectra: int):
+        """fengine_process_host: host buffers (numpy or pinned torch tensors); synchronous."""
+        def hp(x):
+            if isinstance(x, np.ndarray):
+                return x.ctypes.data
+            return x.data_ptr()
+        self._check(self._lib.fengine_process_host(self._h, hp(inp_host), hp(out_host), n_spectra))
+
+    def debug_unpack(self, inp, out_i16, n_spectra: int, stream=None):
+        self._check(self._lib.fengine_debug_unpack(self._h, _dev_ptr(inp), _dev_ptr(out_i16), n_spectra,
+                                                   _stream_handle(stream)))
+
+    def debug_fir(self, inp, out_f32, n_spectra: int, stream=None):
+        self._check(self._lib.fengine_debug_fir(self._h, _dev_ptr(inp), _dev_ptr(out_f32), n_spectra,
+                                                _stream_handle(stream)))
+
+    def last_launch_count(self) -> int:
+        return int(self._lib.fengine_last_launch_count(self._h))

@@ -1,0 +1,88 @@
+// fe_common.cuh -- shared device helpers for the F-engine kernels (sm_100a only).
+//
+// Packed FP32 arithmetic: Blackwell's FFMA2 / FADD2 / FMUL2 (PTX fma.rn.f32x2 etc.) process two
+// floats per issue slot.  The FP32 pipe does 128 FMA lanes/clk/SM either way (measured), so the
+// packed forms do not add flops; they halve the issue slots the arithmetic needs and leave room
+// for the integer unpack, loads/stores and shared-memory traffic.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#if defined(__CUDA_ARCH__) && (__CUDA_ARCH__ < 1000)
+#error "fengine kernels are written for sm_100a (B200) only"
+#endif
+
+namespace fe {
+
+struct f2 {
+    float2 v;
+    __device__ __forceinline__ f2() {}
+    __device__ __forceinline__ f2(float2 x) : v(x) {}
+    __device__ __forceinline__ f2(float a, float b) : v(make_float2(a, b)) {}
+    __device__ __forceinline__ explicit f2(float a) : v(make_float2(a, a)) {}
+};
+__device__ __forceinline__ f2 operator+(f2 a, f2 b) { return f2(__fadd2_rn(a.v, b.v)); }
+__device__ __forceinline__ f2 operator-(f2 a, f2 b) { return f2(__fadd2_rn(a.v, make_float2(-b.v.x, -b.v.y))); }
+__device__ __forceinline__ f2 operator*(f2 a, f2 b) { return f2(__fmul2_rn(a.v, b.v)); }
+__device__ __forceinline__ f2 operator-(f2 a) { return f2(make_float2(-a.v.x, -a.v.y)); }
+// a*b + c and -a*b + c
+__device__ __forceinline__ f2 fma_(f2 a, f2 b, f2 c) { return f2(__ffma2_rn(a.v, b.v, c.v)); }
+__device__ __forceinline__ f2 fnma_(f2 a, f2 b, f2 c) { return f2(__ffma2_rn(make_float2(-a.v.x, -a.v.y), b.v, c.v)); }
+__device__ __forceinline__ f2 scale_(f2 a, float s) { return f2(__fmul2_rn(a.v, make_float2(s, s))); }
+
+// packed value times a scalar (broadcast to both lanes)
+__device__ __forceinline__ f2 operator*(f2 a, float s) { return f2(__fmul2_rn(a.v, make_float2(s, s))); }
+__device__ __forceinline__ f2 fma_(f2 a, float s, f2 c) { return f2(__ffma2_rn(a.v, make_float2(s, s), c.v)); }
+__device__ __forceinline__ f2 fnma_(f2 a, float s, f2 c) { return f2(__ffma2_rn(make_float2(-a.v.x, -a.v.y), make_float2(s, s), c.v)); }
+
+__device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ float fnma_(float a, float b, float c) { return fmaf(-a, b, c); }
+__device__ __forceinline__ float scale_(float a, float s) { return a * s; }
+
+// Complex value over V = float (one point) or f2 (two points in the two packed lanes).
+template <typename V>
+struct cx {
+    V re, im;
+};
+
+template <typename V>
+__device__ __forceinline__ cx<V> cadd(cx<V> a, cx<V> b) { return {a.re + b.re, a.im + b.im}; }
+template <typename V>
+__device__ __forceinline__ cx<V> csub(cx<V> a, cx<V> b) { return {a.re - b.re, a.im - b.im}; }
+// a * (wr + i wi)
+template <typename V, typename W>
+__device__ __forceinline__ cx<V> cmul(cx<V> a, W wr, W wi)
+{
+    cx<V> r;
+    r.re = fnma_(a.im, wi, a.re * wr);
+    r.im = fma_(a.im, wr, a.re * wi);
+    return r;
+}
+// multiply by -i:  (re + i im)(-i) = im - i re
+template <typename V>
+__device__ __forceinline__ cx<V> mul_neg_i(cx<V> a) { return {a.im, -a.re}; }
+
+// streaming global accesses that should not displace the L1-resident tables
+__device__ __forceinline__ float4 ldg_stream_f4(const float4 *p)
+{
+    float4 v;
+    asm volatile("ld.global.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
+                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void stg_stream_f4(float4 *p, float4 v)
+{
+    asm volatile("st.global.L1::no_allocate.v4.f32 [%0], {%1,%2,%3,%4};"
+                 :: "l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+__device__ __forceinline__ void stg_stream_u4(uint4 *p, uint4 v)
+{
+    asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};"
+                 :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+// floor division / modulus by a positive power of two given as log2
+__device__ __host__ __forceinline__ int64_t floor_div_pow2(int64_t x, int lg) { return x >> lg; }
+__device__ __host__ __forceinline__ int64_t floor_mod_pow2(int64_t x, int lg) { return x & ((int64_t(1) << lg) - 1); }
+
+}  // namespace fe

@@ -1,0 +1,132 @@
+// fe_generic.cuh -- simple one-thread-per-output CUDA kernels.
+//
+// They serve (a) the debug hooks of include/fengine.h, (b) shapes the tiled kernels do not cover
+// (tiny n used by brute-force parity tests, tap counts other than 2/4/8/16, n = 2^k not in the
+// plan list).  They are still the CUDA path (no CPU fallback), just not the fast one.
+#pragma once
+#include "fe_common.cuh"
+
+namespace fe {
+
+// sample u of a packed stream (big-endian bit stream), 0 outside [0, L)
+__device__ __forceinline__ int gen_sample(const uint8_t *s, int64_t L, int64_t u)
+{
+    if (u < 0 || u >= L) return 0;
+    const int64_t bit = 10 * u;
+    const uint8_t *b = s + (bit >> 3);
+    const int off = (int)(bit & 7);
+    const uint32_t w = ((uint32_t)b[0] << 8) | (uint32_t)b[1];      // 16-bit window holding the 10 bits
+    const int v = (int)((w >> (6 - off)) & 0x3FFu);
+    return (v ^ 512) - 512;
+}
+
+struct GenParams {
+    const uint8_t *in;
+    const float *weights;
+    const int32_t *coarse;
+    const float *fine_d, *fine_phi;
+    const float2 *gains;
+    int64_t n_coarse, n_fine;
+    int64_t stream_bytes, L, n_spectra;
+    int N, T, P, A;
+};
+
+// debug: window samples [A][P][S][N*T] int16
+__global__ void gen_unpack_kernel(const GenParams p, int16_t *out)
+{
+    const int64_t NT = (int64_t)p.N * p.T;
+    const int64_t total = (int64_t)p.A * p.P * p.n_spectra * NT;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+         idx += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t i = idx % NT;
+        const int64_t m = (idx / NT) % p.n_spectra;
+        const int64_t st = idx / NT / p.n_spectra;
+        const int64_t c = p.coarse[st * p.n_coarse + (p.n_coarse == 1 ? 0 : m)];
+        out[idx] = (int16_t)gen_sample(p.in + st * p.stream_bytes, p.L, (int64_t)p.N * m - c + i);
+    }
+}
+
+// Eq. (1), natural column order: g [A][P][S][N]
+__global__ void gen_fir_kernel(const GenParams p, float *g)
+{
+    const int64_t total = (int64_t)p.A * p.P * p.n_spectra * p.N;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+         idx += (int64_t)gridDim.x * blockDim.x) {
+        const int t = (int)(idx % p.N);
+        const int64_t m = (idx / p.N) % p.n_spectra;
+        const int64_t st = idx / p.N / p.n_spectra;
+        const int64_t c = p.coarse[st * p.n_coarse + (p.n_coarse == 1 ? 0 : m)];
+        const uint8_t *s = p.in + st * p.stream_bytes;
+        float acc = 0.f;
+        for (int j = 0; j < p.T; ++j) {
+            const int64_t u = (int64_t)p.N * (m + j) - c + t;
+            acc = fmaf((float)gen_sample(s, p.L, u), p.weights[t + (int64_t)p.N * j], acc);
+        }
+        g[idx] = acc;
+    }
+}
+
+// N-point DFT of g (natural order, [A][P][S][N]) + rotation + gain (+ quantise): one thread per channel
+template <bool F32OUT>
+__global__ void gen_dft_kernel(const GenParams p, const float *g, int8_t *out, float *out_f32)
+{
+    const int n = p.N / 2;
+    const int64_t total = (int64_t)p.A * p.P * p.n_spectra * n;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+         idx += (int64_t)gridDim.x * blockDim.x) {
+        const int k = (int)(idx % n);
+        const int64_t m = (idx / n) % p.n_spectra;
+        const int64_t st = idx / n / p.n_spectra;
+        const int a = (int)(st / p.P), pol = (int)(st % p.P);
+        const float *row = g + (st * p.n_spectra + m) * p.N;
+        double xr = 0.0, xi = 0.0;
+        for (int t = 0; t < p.N; ++t) {
+            const int e = (int)(((int64_t)k * t) % p.N);
+            double s, c;
+            sincospi(-2.0 * (double)e / (double)p.N, &s, &c);
+            xr += (double)row[t] * c;
+            xi += (double)row[t] * s;
+        }
+        const double d = (double)p.fine_d[st * p.n_fine + (p.n_fine == 1 ? 0 : m)];
+        const double phi = (double)p.fine_phi[st * p.n_fine + (p.n_fine == 1 ? 0 : m)];
+        double s1, c1, s2, c2;
+        sincospi(-2.0 * d * (double)k / (double)p.N, &s1, &c1);
+        sincos(phi, &s2, &c2);
+        const double rr = c1 * c2 - s1 * s2, ri = c1 * s2 + s1 * c2;
+        const double ur = xr * rr - xi * ri, ui = xr * ri + xi * rr;
+        const float2 G = p.gains[st * n + k];
+        const float yr = (float)(ur * (double)G.x - ui * (double)G.y);
+        const float yi = (float)(ur * (double)G.y + ui * (double)G.x);
+        const int64_t o = ((((int64_t)a * p.n_spectra + m) * n + k) * p.P + pol) * 2;
+        if (F32OUT) {
+            out_f32[o] = yr;
+            out_f32[o + 1] = yi;
+        } else {
+            out[o] = (int8_t)__float2int_rn(fminf(fmaxf(yr, -127.f), 127.f));
+            out[o + 1] = (int8_t)__float2int_rn(fminf(fmaxf(yi, -127.f), 127.f));
+        }
+    }
+}
+
+// debug: undo the rotation and the quad permutation of the tiled FIR's scratch rows:
+// g_out [A][P][S][N] (natural) from g' rows ((a*cap + m)*P + p)
+__global__ void unrotate_kernel(const float *gp, float *g_out, const int32_t *coarse, int64_t n_coarse,
+                                int64_t n_spectra, int64_t cap, int N, int P, int A)
+{
+    const int64_t total = (int64_t)A * P * n_spectra * N;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+         idx += (int64_t)gridDim.x * blockDim.x) {
+        const int t = (int)(idx % N);
+        const int64_t m = (idx / N) % n_spectra;
+        const int64_t st = idx / N / n_spectra;
+        const int a = (int)(st / P), pol = (int)(st % P);
+        const int64_t c = coarse[st * n_coarse + (n_coarse == 1 ? 0 : m)];
+        const int cr = (int)(c & (int64_t)(N - 1));
+        const int v = (t - cr) & (N - 1);
+        const int i = v & 3;
+        const int pos = (v & ~3) + (i == 1 ? 2 : i == 2 ? 1 : i);      // stored as (g0, g2, g1, g3)
+        g_out[idx] = gp[(((int64_t)a * cap + m) * P + pol) * N + pos];
+    }
+}
+
+}  // namespace fe

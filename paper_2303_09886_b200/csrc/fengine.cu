@@ -1,0 +1,557 @@
+// fengine.cu -- host side of the C ABI declared in include/fengine.h.
+//
+// Owns the device tables of one engine, validates arguments, and enqueues the kernels of
+// fe_fir.cuh / fe_fft.cuh (tiled path) or fe_generic.cuh (shapes the tiled path does not cover)
+// on the caller's stream.  No arithmetic of the method runs on the host: twiddle tables, the
+// combined rotation*gain table and every step of the path are computed by CUDA kernels.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/fengine.h"
+#include "fe_common.cuh"
+#include "fe_fft.cuh"
+#include "fe_fir.cuh"
+#include "fe_generic.cuh"
+
+using namespace fe;
+
+struct fengine {
+    int A = 0, n = 0, N = 0, lgN = 0, T = 0, P = 0;
+    bool tiled = false;             // tiled kernels cover this (n, T)
+    int64_t n_coarse = 1, n_fine = 1;
+    // device tables
+    float *d_weights = nullptr;
+    int32_t *d_coarse = nullptr;
+    float *d_fine_d = nullptr, *d_fine_phi = nullptr;
+    float2 *d_gains = nullptr, *d_rg = nullptr;
+    float4 *d_tw[3] = {nullptr, nullptr, nullptr};
+    float2 *d_tpost = nullptr;
+    // scratch
+    float *d_scratch = nullptr;
+    size_t scratch_floats = 0;
+    bool rg_dirty = true;
+    // staging for fengine_process_host
+    uint8_t *d_stage_in = nullptr;
+    int8_t *d_stage_out = nullptr;
+    size_t stage_in_bytes = 0, stage_out_bytes = 0;
+    cudaStream_t host_stream = nullptr;
+    // options
+    int64_t chunk_spectra = 0;      // 0 = whole call in one chunk
+    int fir_rows = 64;
+    int64_t last_launches = 0;
+    std::string err;
+};
+
+namespace {
+
+int fail(fengine *fe, int code, const char *fmt, ...)
+{
+    if (fe) {
+        char buf[512];
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(buf, sizeof buf, fmt, ap);
+        va_end(ap);
+        fe->err = buf;
+    }
+    return code;
+}
+
+#define FE_CUDA(fe, call)                                                                       \
+    do {                                                                                        \
+        cudaError_t e_ = (call);                                                                \
+        if (e_ != cudaSuccess)                                                                  \
+            return fail(fe, FENGINE_ERR_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_)); \
+    } while (0)
+
+bool all_finite(const float *p, size_t count)
+{
+    for (size_t i = 0; i < count; ++i)
+        if (!std::isfinite(p[i])) return false;
+    return true;
+}
+
+// ---- plan list of the tiled FFT: <n, passes, R1, R2, R3, R4, threads per pol-FFT> ----
+using Plan1024 = FftPlan<1024, 3, 8, 8, 16, 1, 64>;
+using Plan2048 = FftPlan<2048, 3, 8, 16, 16, 1, 64>;
+using Plan4096 = FftPlan<4096, 3, 16, 16, 16, 1, 128>;
+using Plan8192 = FftPlan<8192, 4, 8, 8, 8, 16, 256>;
+
+bool tiled_n(int n) { return n == 1024 || n == 2048 || n == 4096 || n == 8192; }
+bool tiled_T(int T) { return T == 2 || T == 4 || T == 8 || T == 16; }
+
+template <class Plan>
+int build_tables(fengine *fe)
+{
+    for (int p = 1; p < Plan::q; ++p) {
+        const int R = Plan::radix(p), S = Plan::S(p), M = Plan::M(p - 1);
+        FE_CUDA(fe, cudaMalloc(&fe->d_tw[p - 1], sizeof(float4) * (size_t)R * S));
+        build_pass_twiddles<<<(R * S + 255) / 256, 256>>>(fe->d_tw[p - 1], R, S, M);
+    }
+    FE_CUDA(fe, cudaMalloc(&fe->d_tpost, sizeof(float2) * (size_t)Plan::n));
+    build_post_twiddles<<<(Plan::n + 255) / 256, 256>>>(fe->d_tpost, Plan::n);
+    FE_CUDA(fe, cudaGetLastError());
+    return FENGINE_OK;
+}
+
+template <class Plan, bool F32OUT>
+int launch_fft(fengine *fe, const FftParams &prm, int64_t chunk_len, cudaStream_t stream)
+{
+    const size_t smem = fft_smem_bytes<Plan>(fe->P);
+    const size_t smem_max = fft_smem_bytes<Plan>(2);
+    static bool attr_set = false;
+    if (!attr_set) {
+        FE_CUDA(fe, cudaFuncSetAttribute(fft_kernel<Plan, F32OUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max));
+        attr_set = true;
+    }
+    dim3 grid((unsigned)chunk_len, (unsigned)fe->A);
+    fft_kernel<Plan, F32OUT><<<grid, Plan::tpf * fe->P, smem, stream>>>(prm);
+    return FENGINE_OK;
+}
+
+template <bool F32OUT>
+int launch_fft_n(fengine *fe, const FftParams &prm, int64_t chunk_len, cudaStream_t stream)
+{
+    switch (fe->n) {
+    case 1024: return launch_fft<Plan1024, F32OUT>(fe, prm, chunk_len, stream);
+    case 2048: return launch_fft<Plan2048, F32OUT>(fe, prm, chunk_len, stream);
+    case 4096: return launch_fft<Plan4096, F32OUT>(fe, prm, chunk_len, stream);
+    case 8192: return launch_fft<Plan8192, F32OUT>(fe, prm, chunk_len, stream);
+    }
+    return fail(fe, FENGINE_ERR_INVALID_ARG, "no tiled FFT plan for n=%d", fe->n);
+}
+
+int launch_fir(fengine *fe, const FirParams &prm, int64_t chunk_len, cudaStream_t stream)
+{
+    dim3 grid((unsigned)(fe->N / kFirColsPerBlock), (unsigned)((chunk_len + prm.rows_per_tile - 1) / prm.rows_per_tile),
+              (unsigned)(fe->A * fe->P));
+    switch (fe->T) {
+    case 2: fir_kernel<2, 2><<<grid, kFirThreads, 0, stream>>>(prm); break;
+    case 4: fir_kernel<4, 4><<<grid, kFirThreads, 0, stream>>>(prm); break;
+    case 8: fir_kernel<8, 4><<<grid, kFirThreads, 0, stream>>>(prm); break;
+    case 16: fir_kernel<16, 4><<<grid, kFirThreads, 0, stream>>>(prm); break;
+    default: return fail(fe, FENGINE_ERR_INVALID_ARG, "no tiled FIR for T=%d", fe->T);
+    }
+    return FENGINE_OK;
+}
+
+int ensure_scratch(fengine *fe, size_t floats)
+{
+    if (floats <= fe->scratch_floats) return FENGINE_OK;
+    if (fe->d_scratch) {
+        FE_CUDA(fe, cudaDeviceSynchronize());
+        cudaFree(fe->d_scratch);
+        fe->d_scratch = nullptr;
+        fe->scratch_floats = 0;
+    }
+    if (cudaMalloc(&fe->d_scratch, floats * sizeof(float)) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(fe, FENGINE_ERR_ALLOC, "cannot allocate %zu bytes of scratch", floats * sizeof(float));
+    }
+    fe->scratch_floats = floats;
+    return FENGINE_OK;
+}
+
+GenParams gen_params(const fengine *fe, const void *in, int64_t S)
+{
+    GenParams g{};
+    g.in = static_cast<const uint8_t *>(in);
+    g.weights = fe->d_weights;
+    g.coarse = fe->d_coarse;
+    g.fine_d = fe->d_fine_d;
+    g.fine_phi = fe->d_fine_phi;
+    g.gains = fe->d_gains;
+    g.n_coarse = fe->n_coarse;
+    g.n_fine = fe->n_fine;
+    g.L = (int64_t)fe->N * (S + fe->T - 1);
+    g.stream_bytes = g.L / 4 * 5;
+    g.n_spectra = S;
+    g.N = fe->N;
+    g.T = fe->T;
+    g.P = fe->P;
+    g.A = fe->A;
+    return g;
+}
+
+unsigned gen_grid(int64_t total) { return (unsigned)std::min<int64_t>((total + 255) / 256, 148 * 16); }
+
+int check_call(fengine *fe, const void *in, const void *out, int64_t S)
+{
+    if (!fe) return FENGINE_ERR_INVALID_ARG;
+    fe->err.clear();
+    if (S < 0) return fail(fe, FENGINE_ERR_INVALID_ARG, "n_spectra < 0");
+    if (S == 0) return FENGINE_OK;
+    if (!in || !out) return fail(fe, FENGINE_ERR_INVALID_ARG, "null device pointer");
+    if ((reinterpret_cast<uintptr_t>(in) & 15) || (reinterpret_cast<uintptr_t>(out) & 15))
+        return fail(fe, FENGINE_ERR_INVALID_ARG, "in/out must be 16-byte aligned");
+    if (fe->n_coarse != 1 && fe->n_coarse < S)
+        return fail(fe, FENGINE_ERR_STATE, "coarse delay table has %lld entries per stream, need %lld",
+                    (long long)fe->n_coarse, (long long)S);
+    if (fe->n_fine != 1 && fe->n_fine < S)
+        return fail(fe, FENGINE_ERR_STATE, "fine delay table has %lld entries per stream, need %lld",
+                    (long long)fe->n_fine, (long long)S);
+    return FENGINE_OK;
+}
+
+// the whole path; exactly one of out / out_f32 is non-null
+int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64_t S, cudaStream_t stream)
+{
+    fe->last_launches = 0;
+    if (S == 0) return FENGINE_OK;
+    const int streams = fe->A * fe->P;
+
+    if (!fe->tiled) {
+        int rc = ensure_scratch(fe, (size_t)streams * S * fe->N);
+        if (rc) return rc;
+        const GenParams gp = gen_params(fe, in, S);
+        gen_fir_kernel<<<gen_grid((int64_t)streams * S * fe->N), 256, 0, stream>>>(gp, fe->d_scratch);
+        if (out_f32)
+            gen_dft_kernel<true><<<gen_grid((int64_t)streams * S * fe->n), 256, 0, stream>>>(gp, fe->d_scratch, nullptr, out_f32);
+        else
+            gen_dft_kernel<false><<<gen_grid((int64_t)streams * S * fe->n), 256, 0, stream>>>(gp, fe->d_scratch, out, nullptr);
+        fe->last_launches = 2;
+        FE_CUDA(fe, cudaGetLastError());
+        return FENGINE_OK;
+    }
+
+    const bool per_spectrum = fe->n_coarse != 1 || fe->n_fine != 1;
+    if (!per_spectrum && fe->rg_dirty) {
+        dim3 grid((unsigned)((fe->n + 255) / 256), (unsigned)streams);
+        build_rg_table<<<grid, 256, 0, stream>>>(fe->d_rg, fe->d_gains, fe->d_coarse, fe->d_fine_d, fe->d_fine_phi,
+                                                fe->n, streams);
+        fe->rg_dirty = false;
+        ++fe->last_launches;
+    }
+
+    const int64_t chunk = fe->chunk_spectra > 0 ? std::min<int64_t>(fe->chunk_spectra, S) : S;
+    int rc = ensure_scratch(fe, (size_t)streams * chunk * fe->N);
+    if (rc) return rc;
+
+    FirParams fp{};
+    fp.in = static_cast<const uint8_t *>(in);
+    fp.weights = fe->d_weights;
+    fp.g = fe->d_scratch;
+    fp.coarse = fe->d_coarse;
+    fp.n_coarse = fe->n_coarse;
+    fp.rows_in = S + fe->T - 1;
+    fp.stream_bytes = (int64_t)fe->N * fp.rows_in / 4 * 5;
+    fp.chunk_cap = chunk;
+    fp.lgN = fe->lgN;
+    fp.P = fe->P;
+    fp.rows_per_tile = fe->fir_rows;
+
+    FftParams xp{};
+    xp.g = fe->d_scratch;
+    xp.out = out;
+    xp.out_f32 = out_f32;
+    xp.tab.tw[0] = fe->d_tw[0];
+    xp.tab.tw[1] = fe->d_tw[1];
+    xp.tab.tw[2] = fe->d_tw[2];
+    xp.tab.tpost = fe->d_tpost;
+    xp.rg = fe->d_rg;
+    xp.gains = fe->d_gains;
+    xp.coarse = fe->d_coarse;
+    xp.fine_d = fe->d_fine_d;
+    xp.fine_phi = fe->d_fine_phi;
+    xp.n_coarse = fe->n_coarse;
+    xp.n_fine = fe->n_fine;
+    xp.chunk_cap = chunk;
+    xp.n_spectra = S;
+    xp.P = fe->P;
+    xp.per_spectrum = per_spectrum ? 1 : 0;
+
+    for (int64_t m0 = 0; m0 < S; m0 += chunk) {
+        const int64_t m1 = std::min(S, m0 + chunk);
+        fp.m_begin = xp.m_begin = m0;
+        fp.m_end = xp.m_end = m1;
+        rc = launch_fir(fe, fp, m1 - m0, stream);
+        if (rc) return rc;
+        rc = out_f32 ? launch_fft_n<true>(fe, xp, m1 - m0, stream) : launch_fft_n<false>(fe, xp, m1 - m0, stream);
+        if (rc) return rc;
+        fe->last_launches += 2;
+    }
+    FE_CUDA(fe, cudaGetLastError());
+    return FENGINE_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+fengine_t *fengine_create_batched(int n_antennas, int n_channels, int taps, int n_pols, const float *weights)
+{
+    if (n_antennas < 1 || n_channels < 8 || n_channels > 32768 || (n_channels & (n_channels - 1)) || taps < 1 ||
+        taps > 32 || (n_pols != 1 && n_pols != 2) || !weights)
+        return nullptr;
+    const int N = 2 * n_channels;
+    if (!all_finite(weights, (size_t)N * taps)) return nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return nullptr;                                     // no CPU fallback
+    }
+    fengine *fe = new (std::nothrow) fengine;
+    if (!fe) return nullptr;
+    fe->A = n_antennas;
+    fe->n = n_channels;
+    fe->N = N;
+    fe->T = taps;
+    fe->P = n_pols;
+    while ((1 << fe->lgN) < N) ++fe->lgN;
+    fe->tiled = tiled_n(fe->n) && tiled_T(fe->T);
+    const size_t streams = (size_t)fe->A * fe->P;
+
+    bool ok = cudaMalloc(&fe->d_weights, sizeof(float) * (size_t)N * taps) == cudaSuccess &&
+              cudaMalloc(&fe->d_coarse, sizeof(int32_t) * streams) == cudaSuccess &&
+              cudaMalloc(&fe->d_fine_d, sizeof(float) * streams) == cudaSuccess &&
+              cudaMalloc(&fe->d_fine_phi, sizeof(float) * streams) == cudaSuccess &&
+              cudaMalloc(&fe->d_gains, sizeof(float2) * streams * fe->n) == cudaSuccess &&
+              cudaMalloc(&fe->d_rg, sizeof(float2) * streams * fe->n) == cudaSuccess;
+    if (ok) {
+        std::vector<float2> ones(streams * fe->n, make_float2(1.f, 0.f));
+        ok = cudaMemcpy(fe->d_weights, weights, sizeof(float) * (size_t)N * taps, cudaMemcpyHostToDevice) == cudaSuccess &&
+             cudaMemset(fe->d_coarse, 0, sizeof(int32_t) * streams) == cudaSuccess &&
+             cudaMemset(fe->d_fine_d, 0, sizeof(float) * streams) == cudaSuccess &&
+             cudaMemset(fe->d_fine_phi, 0, sizeof(float) * streams) == cudaSuccess &&
+             cudaMemcpy(fe->d_gains, ones.data(), sizeof(float2) * ones.size(), cudaMemcpyHostToDevice) == cudaSuccess;
+    }
+    if (ok && fe->tiled) {
+        int rc = FENGINE_OK;
+        switch (fe->n) {
+        case 1024: rc = build_tables<Plan1024>(fe); break;
+        case 2048: rc = build_tables<Plan2048>(fe); break;
+        case 4096: rc = build_tables<Plan4096>(fe); break;
+        case 8192: rc = build_tables<Plan8192>(fe); break;
+        }
+        ok = rc == FENGINE_OK;
+    }
+    if (ok) ok = cudaDeviceSynchronize() == cudaSuccess;
+    if (!ok) {
+        cudaGetLastError();
+        fengine_destroy(fe);
+        return nullptr;
+    }
+    return fe;
+}
+
+fengine_t *fengine_create(int n_channels, int taps, int n_pols, const float *weights)
+{
+    return fengine_create_batched(1, n_channels, taps, n_pols, weights);
+}
+
+void fengine_destroy(fengine_t *fe)
+{
+    if (!fe) return;
+    cudaDeviceSynchronize();
+    cudaFree(fe->d_weights);
+    cudaFree(fe->d_coarse);
+    cudaFree(fe->d_fine_d);
+    cudaFree(fe->d_fine_phi);
+    cudaFree(fe->d_gains);
+    cudaFree(fe->d_rg);
+    for (auto &t : fe->d_tw) cudaFree(t);
+    cudaFree(fe->d_tpost);
+    cudaFree(fe->d_scratch);
+    cudaFree(fe->d_stage_in);
+    cudaFree(fe->d_stage_out);
+    if (fe->host_stream) cudaStreamDestroy(fe->host_stream);
+    cudaGetLastError();
+    delete fe;
+}
+
+int fengine_set_coarse_delays(fengine_t *fe, const int32_t *c, int64_t n_per_stream)
+{
+    if (!fe) return FENGINE_ERR_INVALID_ARG;
+    fe->err.clear();
+    if (!c || n_per_stream < 1) return fail(fe, FENGINE_ERR_INVALID_ARG, "bad coarse delay table");
+    const size_t count = (size_t)fe->A * fe->P * n_per_stream;
+    FE_CUDA(fe, cudaDeviceSynchronize());
+    if (n_per_stream != fe->n_coarse) {
+        int32_t *nd = nullptr;
+        if (cudaMalloc(&nd, sizeof(int32_t) * count) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(fe, FENGINE_ERR_ALLOC, "coarse delay table allocation failed");
+        }
+        cudaFree(fe->d_coarse);
+        fe->d_coarse = nd;
+        fe->n_coarse = n_per_stream;
+    }
+    FE_CUDA(fe, cudaMemcpy(fe->d_coarse, c, sizeof(int32_t) * count, cudaMemcpyHostToDevice));
+    fe->rg_dirty = true;
+    return FENGINE_OK;
+}
+
+int fengine_set_fine_delays(fengine_t *fe, const float *delay, const float *phase, int64_t n_per_stream)
+{
+    if (!fe) return FENGINE_ERR_INVALID_ARG;
+    fe->err.clear();
+    if (!delay || !phase || n_per_stream < 1) return fail(fe, FENGINE_ERR_INVALID_ARG, "bad fine delay table");
+    const size_t count = (size_t)fe->A * fe->P * n_per_stream;
+    if (!all_finite(delay, count) || !all_finite(phase, count))
+        return fail(fe, FENGINE_ERR_INVALID_ARG, "non-finite fine delay or phase");
+    FE_CUDA(fe, cudaDeviceSynchronize());
+    if (n_per_stream != fe->n_fine) {
+        float *nd = nullptr, *np = nullptr;
+        if (cudaMalloc(&nd, sizeof(float) * count) != cudaSuccess || cudaMalloc(&np, sizeof(float) * count) != cudaSuccess) {
+            cudaGetLastError();
+            cudaFree(nd);
+            return fail(fe, FENGINE_ERR_ALLOC, "fine delay table allocation failed");
+        }
+        cudaFree(fe->d_fine_d);
+        cudaFree(fe->d_fine_phi);
+        fe->d_fine_d = nd;
+        fe->d_fine_phi = np;
+        fe->n_fine = n_per_stream;
+    }
+    FE_CUDA(fe, cudaMemcpy(fe->d_fine_d, delay, sizeof(float) * count, cudaMemcpyHostToDevice));
+    FE_CUDA(fe, cudaMemcpy(fe->d_fine_phi, phase, sizeof(float) * count, cudaMemcpyHostToDevice));
+    fe->rg_dirty = true;
+    return FENGINE_OK;
+}
+
+int fengine_set_gains(fengine_t *fe, const float *gains_re_im)
+{
+    if (!fe) return FENGINE_ERR_INVALID_ARG;
+    fe->err.clear();
+    if (!gains_re_im) return fail(fe, FENGINE_ERR_INVALID_ARG, "null gains");
+    const size_t count = (size_t)fe->A * fe->P * fe->n;
+    if (!all_finite(gains_re_im, count * 2)) return fail(fe, FENGINE_ERR_INVALID_ARG, "non-finite gain");
+    FE_CUDA(fe, cudaDeviceSynchronize());
+    FE_CUDA(fe, cudaMemcpy(fe->d_gains, gains_re_im, sizeof(float2) * count, cudaMemcpyHostToDevice));
+    fe->rg_dirty = true;
+    return FENGINE_OK;
+}
+
+int fengine_process(fengine_t *fe, const void *in, void *out, int64_t n_spectra, void *stream)
+{
+    int rc = check_call(fe, in, out, n_spectra);
+    if (rc) return rc;
+    return process_impl(fe, in, static_cast<int8_t *>(out), nullptr, n_spectra, static_cast<cudaStream_t>(stream));
+}
+
+int fengine_process_host(fengine_t *fe, const void *in_host, void *out_host, int64_t n_spectra)
+{
+    if (!fe) return FENGINE_ERR_INVALID_ARG;
+    fe->err.clear();
+    if (n_spectra < 0) return fail(fe, FENGINE_ERR_INVALID_ARG, "n_spectra < 0");
+    if (n_spectra == 0) return FENGINE_OK;
+    if (!in_host || !out_host) return fail(fe, FENGINE_ERR_INVALID_ARG, "null host pointer");
+    const size_t in_bytes = (size_t)fe->A * fe->P * ((size_t)fe->N * (n_spectra + fe->T - 1) / 4 * 5);
+    const size_t out_bytes = (size_t)fe->A * n_spectra * fe->n * fe->P * 2;
+    if (!fe->host_stream) FE_CUDA(fe, cudaStreamCreateWithFlags(&fe->host_stream, cudaStreamNonBlocking));
+    if (in_bytes > fe->stage_in_bytes) {
+        cudaFree(fe->d_stage_in);
+        fe->d_stage_in = nullptr;
+        fe->stage_in_bytes = 0;
+        if (cudaMalloc(&fe->d_stage_in, in_bytes) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(fe, FENGINE_ERR_ALLOC, "input staging allocation failed");
+        }
+        fe->stage_in_bytes = in_bytes;
+    }
+    if (out_bytes > fe->stage_out_bytes) {
+        cudaFree(fe->d_stage_out);
+        fe->d_stage_out = nullptr;
+        fe->stage_out_bytes = 0;
+        if (cudaMalloc(&fe->d_stage_out, out_bytes) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(fe, FENGINE_ERR_ALLOC, "output staging allocation failed");
+        }
+        fe->stage_out_bytes = out_bytes;
+    }
+    FE_CUDA(fe, cudaMemcpyAsync(fe->d_stage_in, in_host, in_bytes, cudaMemcpyHostToDevice, fe->host_stream));
+    int rc = check_call(fe, fe->d_stage_in, fe->d_stage_out, n_spectra);
+    if (rc) return rc;
+    rc = process_impl(fe, fe->d_stage_in, fe->d_stage_out, nullptr, n_spectra, fe->host_stream);
+    if (rc) return rc;
+    FE_CUDA(fe, cudaMemcpyAsync(out_host, fe->d_stage_out, out_bytes, cudaMemcpyDeviceToHost, fe->host_stream));
+    FE_CUDA(fe, cudaStreamSynchronize(fe->host_stream));
+    return FENGINE_OK;
+}
+
+int fengine_process_f32(fengine_t *fe, const void *in, float *spectra_out, int64_t n_spectra, void *stream)
+{
+    int rc = check_call(fe, in, spectra_out, n_spectra);
+    if (rc) return rc;
+    return process_impl(fe, in, nullptr, spectra_out, n_spectra, static_cast<cudaStream_t>(stream));
+}
+
+int fengine_debug_unpack(fengine_t *fe, const void *in, int16_t *samples_out, int64_t n_spectra, void *stream)
+{
+    int rc = check_call(fe, in, samples_out, n_spectra);
+    if (rc || n_spectra == 0) return rc;
+    const GenParams gp = gen_params(fe, in, n_spectra);
+    const int64_t total = (int64_t)fe->A * fe->P * n_spectra * fe->N * fe->T;
+    gen_unpack_kernel<<<gen_grid(total), 256, 0, static_cast<cudaStream_t>(stream)>>>(gp, samples_out);
+    FE_CUDA(fe, cudaGetLastError());
+    return FENGINE_OK;
+}
+
+int fengine_debug_fir(fengine_t *fe, const void *in, float *g_out, int64_t n_spectra, void *stream)
+{
+    int rc = check_call(fe, in, g_out, n_spectra);
+    if (rc || n_spectra == 0) return rc;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const int64_t total = (int64_t)fe->A * fe->P * n_spectra * fe->N;
+    if (!fe->tiled) {
+        gen_fir_kernel<<<gen_grid(total), 256, 0, s>>>(gen_params(fe, in, n_spectra), g_out);
+    } else {
+        rc = ensure_scratch(fe, (size_t)total);
+        if (rc) return rc;
+        FirParams fp{};
+        fp.in = static_cast<const uint8_t *>(in);
+        fp.weights = fe->d_weights;
+        fp.g = fe->d_scratch;
+        fp.coarse = fe->d_coarse;
+        fp.n_coarse = fe->n_coarse;
+        fp.rows_in = n_spectra + fe->T - 1;
+        fp.stream_bytes = (int64_t)fe->N * fp.rows_in / 4 * 5;
+        fp.m_begin = 0;
+        fp.m_end = n_spectra;
+        fp.chunk_cap = n_spectra;
+        fp.lgN = fe->lgN;
+        fp.P = fe->P;
+        fp.rows_per_tile = fe->fir_rows;
+        rc = launch_fir(fe, fp, n_spectra, s);
+        if (rc) return rc;
+        unrotate_kernel<<<gen_grid(total), 256, 0, s>>>(fe->d_scratch, g_out, fe->d_coarse, fe->n_coarse, n_spectra,
+                                                        n_spectra, fe->N, fe->P, fe->A);
+    }
+    FE_CUDA(fe, cudaGetLastError());
+    return FENGINE_OK;
+}
+
+const char *fengine_last_error(const fengine_t *fe) { return fe ? fe->err.c_str() : "null handle"; }
+
+int fengine_set_option(fengine_t *fe, const char *key, int64_t value)
+{
+    if (!fe || !key) return FENGINE_ERR_INVALID_ARG;
+    fe->err.clear();
+    if (!strcmp(key, "chunk_spectra")) {
+        if (value < 0) return fail(fe, FENGINE_ERR_INVALID_ARG, "chunk_spectra < 0");
+        fe->chunk_spectra = value;
+        return FENGINE_OK;
+    }
+    if (!strcmp(key, "fir_rows")) {
+        if (value < 1 || value > 65536) return fail(fe, FENGINE_ERR_INVALID_ARG, "fir_rows out of range");
+        fe->fir_rows = (int)value;
+        return FENGINE_OK;
+    }
+    if (!strcmp(key, "force_generic")) {
+        fe->tiled = value ? false : (tiled_n(fe->n) && tiled_T(fe->T));
+        return FENGINE_OK;
+    }
+    return fail(fe, FENGINE_ERR_INVALID_ARG, "unknown option %s", key);
+}
+
+int64_t fengine_last_launch_count(const fengine_t *fe) { return fe ? fe->last_launches : 0; }
+
+}  // extern "C"

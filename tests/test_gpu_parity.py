@@ -1,0 +1,333 @@
+"""GPU parity tests (`-m gpu`): the CUDA path, called through the C ABI, against the float64 oracle.
+
+Bars (BASELINE.json north_star; R12, R13):
+  * unpack + coarse delay: bit-exact
+  * pre-quantisation spectra: max-abs error <= 1e-4 x per-stream spectrum RMS
+  * int8 outputs: identical except +-1 LSB on <= 1e-4 of the values
+"""
+import numpy as np
+import pytest
+
+import oracle
+import synth_inputs as si
+
+pytestmark = pytest.mark.gpu
+
+TOL_REL = 1e-4          # x per-stream RMS (north_star)
+INT8_MISMATCH = 1e-4    # fraction allowed to differ by exactly 1 LSB
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+@pytest.fixture(scope="module")
+def fb():
+    import paper_2303_09886_b200 as fb
+    fb.lib()            # fails loudly if the CUDA library is missing
+    return fb
+
+
+def make_engine(fb, w, **opts):
+    fe = fb.FEngine(w.n, w.T, w.P, w.weights, n_antennas=w.A)
+    fe.set_coarse_delays(w.coarse)
+    fe.set_fine_delays(w.fine_delay, w.phase)
+    fe.set_gains(w.gains)
+    for k, v in opts.items():
+        fe.set_option(k, v)
+    return fe
+
+
+def gpu_run(torch, fe, w, want=("int8", "f32")):
+    d_in = torch.from_numpy(w.packed.reshape(-1)).cuda()
+    res = {}
+    if "int8" in want:
+        d_out = torch.full(fe.output_shape(w.S), 99, dtype=torch.int8, device="cuda")
+        fe.process(d_in, d_out, w.S)
+        torch.cuda.synchronize()
+        res["out"] = d_out.cpu().numpy()
+    if "f32" in want:
+        d_y = torch.full(fe.output_shape(w.S), float("nan"), dtype=torch.float32, device="cuda")
+        fe.process_f32(d_in, d_y, w.S)
+        torch.cuda.synchronize()
+        y = d_y.cpu().numpy().astype(np.float64)
+        res["Y"] = y[..., 0] + 1j * y[..., 1]
+    return res
+
+
+def oracle_run(w, sel=None):
+    return oracle.process(w.packed, w.A, w.n, w.T, w.P, w.weights, w.S, coarse=w.coarse, fine_delay=w.fine_delay,
+                          phase=w.phase, gains=w.gains, sel=sel)
+
+
+def check_parity(got, ref, label=""):
+    """Element-by-element comparison at the north-star tolerances; returns the worst figures."""
+    worst = 0.0
+    if "Y" in got:
+        Yg, Yr = got["Y"], ref["Y"]
+        assert Yg.shape == Yr.shape
+        assert np.all(np.isfinite(Yg.real)) and np.all(np.isfinite(Yg.imag)), f"{label}: non-finite output"
+        A, S, n, P = Yr.shape
+        for a in range(A):
+            for p in range(P):
+                rms = np.sqrt(np.mean(np.abs(Yr[a, :, :, p]) ** 2))
+                diff = Yg[a, :, :, p] - Yr[a, :, :, p]
+                err = max(np.abs(diff.real).max(), np.abs(diff.imag).max())
+                worst = max(worst, err / max(rms, 1e-300))
+                assert err <= TOL_REL * rms, f"{label}: stream ({a},{p}) max-abs err {err:.3e} > 1e-4 x RMS {rms:.3e}"
+    if "out" in got:
+        og, orf = got["out"].astype(np.int32), ref["out"].astype(np.int32)
+        assert og.shape == orf.shape
+        d = np.abs(og - orf)
+        assert d.max() <= 1, f"{label}: int8 differs by more than 1 LSB (max {d.max()})"
+        frac = np.count_nonzero(d) / d.size
+        assert frac <= INT8_MISMATCH, f"{label}: {frac:.2e} of int8 values differ"
+        assert og.min() >= -127 and og.max() <= 127
+    return worst
+
+
+# ----------------------------------------------------------------------------------------------
+# unpack + coarse delay: bit-exact
+# ----------------------------------------------------------------------------------------------
+def _oracle_windows(w):
+    out = np.empty((w.A, w.P, w.S, w.N * w.T), dtype=np.int16)
+    for a in range(w.A):
+        for p in range(w.P):
+            s = oracle.unpack10(w.packed[a, p], w.L).astype(np.float64)
+            for m in range(w.S):
+                c = int(w.coarse[a, p, m if w.coarse.shape[2] > 1 else 0])
+                out[a, p, m] = oracle.window(s, w.N, w.T, m, c).astype(np.int16)
+    return out
+
+
+@pytest.mark.parametrize("case", ["config1", "tiny_negative", "per_spectrum"])
+def test_unpack_and_coarse_delay_bit_exact(torch, fb, case):
+    if case == "config1":
+        w = si.make_workload(1, n_spectra=20)
+    elif case == "tiny_negative":
+        w = si.custom_workload(A=2, n=16, T=3, S=7, seed=21, coarse_range=(-40, 70))
+    else:
+        w = si.custom_workload(A=1, n=64, T=4, S=9, seed=22, per_spectrum=True, coarse_range=(-10, 300))
+    fe = make_engine(fb, w)
+    d_in = torch.from_numpy(w.packed.reshape(-1)).cuda()
+    d_s = torch.zeros((w.A, w.P, w.S, w.N * w.T), dtype=torch.int16, device="cuda")
+    fe.debug_unpack(d_in, d_s, w.S)
+    torch.cuda.synchronize()
+    np.testing.assert_array_equal(d_s.cpu().numpy(), _oracle_windows(w))
+
+
+@pytest.mark.parametrize("n,T,c", [(1024, 16, 0), (1024, 16, 3), (4096, 16, 4093), (4096, 8, -5), (2048, 4, 70001),
+                                    (8192, 16, 16382), (1024, 2, 2047)])
+def test_tiled_fir_unpack_is_bit_exact_with_one_hot_weights(torch, fb, n, T, c):
+    """weights = 1 at one tap: the tiled FIR must return the delayed integer samples exactly."""
+    N = 2 * n
+    S = 70
+    w = si.custom_workload(A=1, n=n, T=T, S=S, seed=23)
+    j0 = T // 2
+    h = np.zeros(N * T, dtype=np.float32)
+    h[N * j0:N * (j0 + 1)] = 1.0
+    fe = fb.FEngine(n, T, 2, h, n_antennas=1)
+    fe.set_coarse_delays(np.full((1, 2, 1), c, np.int32))
+    d_in = torch.from_numpy(w.packed.reshape(-1)).cuda()
+    d_g = torch.zeros((1, 2, S, N), dtype=torch.float32, device="cuda")
+    fe.debug_fir(d_in, d_g, S)
+    torch.cuda.synchronize()
+    g = d_g.cpu().numpy()
+    for p in range(2):
+        s = w.samples[0, p].astype(np.int64)
+        idx = N * np.arange(S)[:, None] - c + N * j0 + np.arange(N)[None, :]
+        ok = (idx >= 0) & (idx < s.size)
+        expect = np.where(ok, s[np.clip(idx, 0, s.size - 1)], 0)
+        np.testing.assert_array_equal(g[0, p], expect.astype(np.float32))
+
+
+# ----------------------------------------------------------------------------------------------
+# FIR (Eq. 1) against the oracle's direct sum
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,T,per_spectrum", [(1024, 16, False), (4096, 16, True), (64, 5, False)])
+def test_fir_matches_oracle(torch, fb, n, T, per_spectrum):
+    w = si.custom_workload(A=2, n=n, T=T, S=37, seed=24, per_spectrum=per_spectrum, random_weights=True,
+                           coarse_range=(-7, 2 * n + 50))
+    fe = make_engine(fb, w)
+    d_in = torch.from_numpy(w.packed.reshape(-1)).cuda()
+    d_g = torch.zeros((w.A, w.P, w.S, w.N), dtype=torch.float32, device="cuda")
+    fe.debug_fir(d_in, d_g, w.S)
+    torch.cuda.synchronize()
+    g = d_g.cpu().numpy().astype(np.float64)
+    for a in range(w.A):
+        for p in range(w.P):
+            s = w.samples[a, p].astype(np.float64)
+            for m in range(0, w.S, 5):
+                c = int(w.coarse[a, p, m if per_spectrum else 0])
+                ref = oracle.fir(oracle.window(s, w.N, T, m, c), w.weights, w.N, T)
+                scale = np.sqrt(np.mean(ref ** 2)) + 1e-30
+                assert np.abs(g[a, p, m] - ref).max() <= 5e-6 * scale + 1e-30
+
+
+# ----------------------------------------------------------------------------------------------
+# whole path
+# ----------------------------------------------------------------------------------------------
+def test_config1_full(torch, fb):
+    w = si.make_workload(1)
+    fe = make_engine(fb, w)
+    got = gpu_run(torch, fe, w)
+    ref = oracle_run(w)
+    worst = check_parity(got, ref, "config1")
+    print(f"config1 worst err/RMS = {worst:.3e}")
+    # the saturated tone bin of pin P11
+    np.testing.assert_array_equal(got["out"][0, 64, 100, 0], [127, -127])
+
+
+@pytest.mark.parametrize("cfg,kw", [
+    (2, dict(n_spectra=150)),
+    (2, dict(n_spectra=70, n_antennas=2)),
+    (4, dict(n_spectra=150, n_antennas=2)),
+    (4, dict(n_spectra=130, n_antennas=1, sigma=182.0)),
+    (5, dict(n_spectra=40, n_antennas=3, n_channels=1024)),
+    (5, dict(n_spectra=33, n_antennas=2, n_channels=8192)),
+])
+def test_configs_reduced(torch, fb, cfg, kw):
+    w = si.make_workload(cfg, **kw)
+    fe = make_engine(fb, w)
+    got = gpu_run(torch, fe, w)
+    ref = oracle_run(w)
+    worst = check_parity(got, ref, f"config{cfg} {kw}")
+    print(f"config{cfg} {kw}: worst err/RMS = {worst:.3e}")
+
+
+@pytest.mark.parametrize("n,T,S,A,P,per_spectrum,crange", [
+    (8, 1, 5, 1, 2, False, (0, 16)),
+    (16, 3, 6, 2, 2, True, (-20, 50)),
+    (64, 4, 9, 2, 1, False, (-3, 128)),
+    (256, 16, 4, 1, 2, True, (0, 512)),
+    (512, 7, 3, 1, 2, False, (0, 1024)),
+    (1024, 16, 1, 1, 2, False, (0, 2048)),          # a single spectrum
+    (1024, 8, 67, 3, 1, True, (-2048, 4096)),       # one pol, three antennas, per-spectrum random delays
+    (2048, 4, 65, 1, 2, False, (5, 6)),
+    (4096, 2, 66, 1, 2, False, (8190, 8191)),
+    (4096, 16, 129, 1, 2, False, (-1, 0)),
+])
+def test_shapes_and_edges(torch, fb, n, T, S, A, P, per_spectrum, crange):
+    w = si.custom_workload(A=A, n=n, T=T, S=S, P=P, seed=25, per_spectrum=per_spectrum, random_weights=(n <= 64),
+                           coarse_range=crange)
+    fe = make_engine(fb, w)
+    got = gpu_run(torch, fe, w)
+    ref = oracle_run(w)
+    check_parity(got, ref, f"n={n} T={T} S={S} A={A} P={P}")
+
+
+def test_generic_and_tiled_kernels_agree(torch, fb):
+    w = si.make_workload(1, n_spectra=6)
+    a = gpu_run(torch, make_engine(fb, w), w)
+    b = gpu_run(torch, make_engine(fb, w, force_generic=1), w)
+    ref = oracle_run(w)
+    check_parity(a, ref, "tiled")
+    check_parity(b, ref, "generic")
+
+
+def test_chunking_and_tile_size_do_not_change_results(torch, fb):
+    w = si.make_workload(2, n_spectra=131, n_antennas=2)
+    base = gpu_run(torch, make_engine(fb, w), w, want=("int8",))["out"]
+    for opts in (dict(chunk_spectra=48), dict(chunk_spectra=1), dict(fir_rows=17), dict(chunk_spectra=64, fir_rows=32)):
+        other = gpu_run(torch, make_engine(fb, w, **opts), w, want=("int8",))["out"]
+        np.testing.assert_array_equal(base, other, err_msg=str(opts))
+
+
+def test_saturation_never_produces_minus_128(torch, fb):
+    w = si.make_workload(1, n_spectra=8)
+    w.gains[:] = 1e4
+    fe = make_engine(fb, w)
+    out = gpu_run(torch, fe, w, want=("int8",))["out"]
+    assert out.min() == -127 and out.max() == 127
+    ref = oracle_run(w)
+    check_parity({"out": out}, ref, "saturated")
+
+
+def test_process_host_matches_device_path(torch, fb):
+    w = si.make_workload(1, n_spectra=24)
+    fe = make_engine(fb, w)
+    dev = gpu_run(torch, fe, w, want=("int8",))["out"]
+    host_out = np.zeros(fe.output_shape(w.S), dtype=np.int8)
+    fe.process_host(np.ascontiguousarray(w.packed.reshape(-1)), host_out, w.S)
+    np.testing.assert_array_equal(dev, host_out)
+    pin_in = torch.from_numpy(w.packed.reshape(-1)).pin_memory()
+    pin_out = torch.zeros(fe.output_shape(w.S), dtype=torch.int8).pin_memory()
+    fe.process_host(pin_in, pin_out, w.S)
+    np.testing.assert_array_equal(dev, pin_out.numpy())
+
+
+def test_setters_take_effect_between_calls(torch, fb):
+    w = si.make_workload(1, n_spectra=10)
+    fe = make_engine(fb, w)
+    got1 = gpu_run(torch, fe, w)
+    check_parity(got1, oracle_run(w), "first")
+    w.coarse = np.array([[[17], [2051]]], dtype=np.int32)
+    w.fine_delay = np.full((1, 2, 1), -0.4, np.float32)
+    w.phase = np.full((1, 2, 1), 2.5, np.float32)
+    w.gains = (w.gains * (0.5 - 2j)).astype(np.complex64)
+    fe.set_coarse_delays(w.coarse)
+    fe.set_fine_delays(w.fine_delay, w.phase)
+    fe.set_gains(w.gains)
+    check_parity(gpu_run(torch, fe, w), oracle_run(w), "after setters")
+
+
+def test_argument_errors(torch, fb):
+    w = si.make_workload(1, n_spectra=4)
+    fe = make_engine(fb, w)
+    d_in = torch.from_numpy(w.packed.reshape(-1)).cuda()
+    d_out = torch.zeros(fe.output_shape(w.S), dtype=torch.int8, device="cuda")
+    fe.process(d_in, d_out, 0)                                   # no-op
+    with pytest.raises(fb.FEngineError) as e:
+        fe.process(d_in.data_ptr() + 1, d_out, w.S)              # misaligned
+    assert e.value.code == 1
+    with pytest.raises(fb.FEngineError) as e:
+        fe.process(d_in, d_out, -1)
+    assert e.value.code == 1
+    fe.set_coarse_delays(np.zeros((1, 2, 3), np.int32))          # table shorter than n_spectra
+    with pytest.raises(fb.FEngineError) as e:
+        fe.process(d_in, d_out, w.S)
+    assert e.value.code == 4
+    with pytest.raises(fb.FEngineError) as e:
+        fe.set_gains(np.full((1, 2, w.n), np.nan, np.complex64))
+    assert e.value.code == 1
+    with pytest.raises(fb.FEngineError):
+        fb.FEngine(1000, 16, 2, np.zeros(2000 * 16, np.float32))  # n not a power of two
+    with pytest.raises(fb.FEngineError):
+        fe.set_option("no_such_option", 1)
+
+
+# ----------------------------------------------------------------------------------------------
+# full size, in the launch configuration bench.py times: sampled spectra against the oracle
+# ----------------------------------------------------------------------------------------------
+def test_config2_full_size_sampled(torch, fb):
+    w = si.make_workload(2)                                      # 4 antennas x 2 pols, n=4096, 2^24 samples per pol
+    assert w.S == 2033
+    fe = make_engine(fb, w)
+    d_in = torch.from_numpy(w.packed.reshape(-1)).cuda()
+    d_out = torch.zeros(fe.output_shape(w.S), dtype=torch.int8, device="cuda")
+    d_y = torch.zeros(fe.output_shape(w.S), dtype=torch.float32, device="cuda")
+    fe.process(d_in, d_out, w.S)
+    fe.process_f32(d_in, d_y, w.S)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(5)
+    sel = np.unique(np.concatenate([[0, 1, 14, 15, 16, 63, 64, 2031, 2032], rng.integers(0, w.S, 16)]))
+    ref = oracle_run(w, sel=sel)
+    idx = torch.from_numpy(sel).cuda()
+    y = d_y[:, idx].cpu().numpy().astype(np.float64)
+    got = {"out": d_out[:, idx].cpu().numpy(), "Y": y[..., 0] + 1j * y[..., 1]}
+    worst = check_parity(got, ref, "config2 full size")
+    print(f"config2 full size: worst err/RMS over sampled spectra = {worst:.3e}")
+    # one-by-one definition check (NT-term windowed DTFT) on a few single outputs
+    for _ in range(6):
+        a, p = int(rng.integers(w.A)), int(rng.integers(2))
+        m, k = int(rng.integers(w.S)), int(rng.integers(w.n))
+        yref = oracle.direct_channel(w.packed[a, p], w.L, w.n, w.T, w.weights, m, int(w.coarse[a, p, 0]),
+                                     w.fine_delay[a, p, 0], w.phase[a, p, 0], w.gains[a, p, k], k)
+        yg = d_y[a, m, k, p].cpu().numpy().astype(np.float64)
+        assert abs(complex(yg[0], yg[1]) - yref) < 1e-4 * 30.0   # ~1e-4 x the noise RMS of this config
+    # properties that hold at any size: range, and the output is not left unwritten anywhere
+    assert int(d_out.min()) >= -127 and int(d_out.max()) <= 127
+    assert float(torch.count_nonzero(d_out)) / d_out.numel() > 0.9
