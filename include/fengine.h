@@ -127,9 +127,19 @@ int fengine_debug_unpack(fengine_t *fe, const void *in, int16_t *samples_out, in
 int fengine_debug_fir(fengine_t *fe, const void *in, float *g_out, int64_t n_spectra, void *stream);
 
 /* Tuning knobs (optional; defaults are chosen at create).  key: "chunk_spectra" (spectra per
- * L2-resident chunk; 0 = whole call), "fir_rows" (spectra per FIR tile).  Returns INVALID_ARG for
+ * L2-resident chunk; 0 = whole call), "fir_rows" (spectra per FIR tile), "profile" (0/1, see below), "force_generic" (0/1: use the simple
+ * one-thread-per-output kernels).  Returns INVALID_ARG for
  * unknown keys. */
 int fengine_set_option(fengine_t *fe, const char *key, int64_t value);
+
+/*
+ * Per-kernel timing for the roofline report.  With option "profile" = 1 every fengine_process call
+ * records CUDA events on the caller's stream around each kernel.  fengine_profile_read waits for
+ * them, returns the summed device time of the FIR kernel launches and of the FFT kernel launches
+ * (milliseconds) and the number of launches of each since the last read, and clears the record.
+ * fir_ms, fft_ms, n_fir, n_fft: HOST out-pointers (any may be NULL).
+ */
+int fengine_profile_read(fengine_t *fe, double *fir_ms, double *fft_ms, int64_t *n_fir, int64_t *n_fft);
 
 /* Number of kernel launches the last fengine_process / _f32 call enqueued (for bench accounting). */
 int64_t fengine_last_launch_count(const fengine_t *fe);

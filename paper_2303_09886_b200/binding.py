@@ -15,7 +15,7 @@ EXPORTED_SYMBOLS = [
     "fengine_create", "fengine_create_batched", "fengine_destroy", "fengine_set_coarse_delays",
     "fengine_set_fine_delays", "fengine_set_gains", "fengine_process", "fengine_process_host",
     "fengine_last_error", "fengine_process_f32", "fengine_debug_unpack", "fengine_debug_fir",
-    "fengine_set_option", "fengine_last_launch_count",
+    "fengine_set_option", "fengine_last_launch_count", "fengine_profile_read",
 ]
 
 STATUS = {0: "OK", 1: "INVALID_ARG", 2: "ALLOC", 3: "CUDA", 4: "STATE"}
@@ -58,6 +58,7 @@ def lib() -> C.CDLL:
         L.fengine_last_error.argtypes = [vp]
         L.fengine_last_error.restype = C.c_char_p
         L.fengine_set_option.argtypes = [vp, C.c_char_p, i64]
+        L.fengine_profile_read.argtypes = [vp, vp, vp, vp, vp]
         L.fengine_last_launch_count.argtypes = [vp]
         L.fengine_last_launch_count.restype = i64
         _lib = L
@@ -166,6 +167,13 @@ class FEngine:
     def debug_fir(self, inp, out_f32, n_spectra: int, stream=None):
         self._check(self._lib.fengine_debug_fir(self._h, _dev_ptr(inp), _dev_ptr(out_f32), n_spectra,
                                                 _stream_handle(stream)))
+
+    def profile_read(self):
+        """(fir_ms, fft_ms, n_fir, n_fft) summed since the last read (option "profile" must be 1)."""
+        a, b = C.c_double(), C.c_double()
+        na, nb = C.c_int64(), C.c_int64()
+        self._check(self._lib.fengine_profile_read(self._h, C.byref(a), C.byref(b), C.byref(na), C.byref(nb)))
+        return a.value, b.value, na.value, nb.value
 
     def last_launch_count(self) -> int:
         return int(self._lib.fengine_last_launch_count(self._h))

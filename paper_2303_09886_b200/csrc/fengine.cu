@@ -47,6 +47,9 @@ struct fengine {
     int64_t chunk_spectra = 0;      // 0 = whole call in one chunk
     int fir_rows = 64;
     int64_t last_launches = 0;
+    bool profile = false;
+    std::vector<cudaEvent_t> ev_pool;       // reused events
+    std::vector<cudaEvent_t> ev_used;       // triplets (before FIR, between, after FFT) in call order
     std::string err;
 };
 
@@ -272,10 +275,25 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
         const int64_t m1 = std::min(S, m0 + chunk);
         fp.m_begin = xp.m_begin = m0;
         fp.m_end = xp.m_end = m1;
+        cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+        if (fe->profile) {
+            for (auto &e : ev) {
+                if (fe->ev_pool.empty()) {
+                    FE_CUDA(fe, cudaEventCreate(&e));
+                } else {
+                    e = fe->ev_pool.back();
+                    fe->ev_pool.pop_back();
+                }
+                fe->ev_used.push_back(e);
+            }
+            FE_CUDA(fe, cudaEventRecord(ev[0], stream));
+        }
         rc = launch_fir(fe, fp, m1 - m0, stream);
         if (rc) return rc;
+        if (fe->profile) FE_CUDA(fe, cudaEventRecord(ev[1], stream));
         rc = out_f32 ? launch_fft_n<true>(fe, xp, m1 - m0, stream) : launch_fft_n<false>(fe, xp, m1 - m0, stream);
         if (rc) return rc;
+        if (fe->profile) FE_CUDA(fe, cudaEventRecord(ev[2], stream));
         fe->last_launches += 2;
     }
     FE_CUDA(fe, cudaGetLastError());
@@ -363,6 +381,8 @@ void fengine_destroy(fengine_t *fe)
     cudaFree(fe->d_stage_in);
     cudaFree(fe->d_stage_out);
     if (fe->host_stream) cudaStreamDestroy(fe->host_stream);
+    for (auto e : fe->ev_pool) cudaEventDestroy(e);
+    for (auto e : fe->ev_used) cudaEventDestroy(e);
     cudaGetLastError();
     delete fe;
 }
@@ -545,11 +565,39 @@ int fengine_set_option(fengine_t *fe, const char *key, int64_t value)
         fe->fir_rows = (int)value;
         return FENGINE_OK;
     }
+    if (!strcmp(key, "profile")) {
+        fe->profile = value != 0;
+        return FENGINE_OK;
+    }
     if (!strcmp(key, "force_generic")) {
         fe->tiled = value ? false : (tiled_n(fe->n) && tiled_T(fe->T));
         return FENGINE_OK;
     }
     return fail(fe, FENGINE_ERR_INVALID_ARG, "unknown option %s", key);
+}
+
+int fengine_profile_read(fengine_t *fe, double *fir_ms, double *fft_ms, int64_t *n_fir, int64_t *n_fft)
+{
+    if (!fe) return FENGINE_ERR_INVALID_ARG;
+    fe->err.clear();
+    double fir = 0.0, fft = 0.0;
+    int64_t count = 0;
+    for (size_t i = 0; i + 2 < fe->ev_used.size(); i += 3) {
+        FE_CUDA(fe, cudaEventSynchronize(fe->ev_used[i + 2]));
+        float a = 0.f, b = 0.f;
+        FE_CUDA(fe, cudaEventElapsedTime(&a, fe->ev_used[i], fe->ev_used[i + 1]));
+        FE_CUDA(fe, cudaEventElapsedTime(&b, fe->ev_used[i + 1], fe->ev_used[i + 2]));
+        fir += a;
+        fft += b;
+        ++count;
+    }
+    for (auto e : fe->ev_used) fe->ev_pool.push_back(e);
+    fe->ev_used.clear();
+    if (fir_ms) *fir_ms = fir;
+    if (fft_ms) *fft_ms = fft;
+    if (n_fir) *n_fir = count;
+    if (n_fft) *n_fft = count;
+    return FENGINE_OK;
 }
 
 int64_t fengine_last_launch_count(const fengine_t *fe) { return fe ? fe->last_launches : 0; }
