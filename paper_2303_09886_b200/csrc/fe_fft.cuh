@@ -372,65 +372,67 @@ __device__ __forceinline__ void fft_pass_last(const float4 *sm, const FftParams 
 template <class Plan>
 constexpr size_t fft_smem_bytes(int P)
 {
-    return (size_t)P * Plan::units * 16 + (size_t)Plan::n * P * 2 + 2 * sizeof(SpectrumPhase);
+    return (size_t)Plan::units * 16 + (size_t)Plan::n * P * 2 + sizeof(SpectrumPhase);
 }
 
+// One CTA per (antenna, spectrum); the pols are transformed one after the other through the same
+// exchange buffer (small CTAs, several per SM, each at a different phase of its spectrum).
 template <class Plan, bool F32OUT>
-__global__ void __launch_bounds__(Plan::tpf * 2) fft_kernel(const FftParams prm)
+__global__ void __launch_bounds__(Plan::tpf, 512 / Plan::tpf) fft_kernel(const FftParams prm)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int n = Plan::n, N = 2 * n;
     const int P = prm.P;
-    float4 *sm_all = reinterpret_cast<float4 *>(smem_raw);
-    uint16_t *stage = reinterpret_cast<uint16_t *>(smem_raw + (size_t)P * Plan::units * 16);
-    SpectrumPhase *sph_all = reinterpret_cast<SpectrumPhase *>(smem_raw + (size_t)P * Plan::units * 16 + (size_t)n * P * 2);
+    float4 *sm = reinterpret_cast<float4 *>(smem_raw);
+    uint16_t *stage = reinterpret_cast<uint16_t *>(smem_raw + (size_t)Plan::units * 16);
+    SpectrumPhase *sph = reinterpret_cast<SpectrumPhase *>(smem_raw + (size_t)Plan::units * 16 + (size_t)n * P * 2);
 
-    const int pol = threadIdx.x / Plan::tpf;
-    const int tid = threadIdx.x - pol * Plan::tpf;
+    const int tid = threadIdx.x;
     const int a = blockIdx.y;
     const int64_t m = prm.m_begin + blockIdx.x;
     if (m >= prm.m_end) return;
-    float4 *sm = sm_all + (size_t)pol * Plan::units;
-    const int64_t st = (int64_t)a * P + pol;
-    const float4 *grow = reinterpret_cast<const float4 *>(
-        prm.g + (((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * P + pol) * (int64_t)N);
 
-    // per-spectrum phasor set-up
-    double dts = 0.0;
-    int cr = 0;
-    SpectrumPhase *sph = sph_all + pol;
-    if (prm.per_spectrum) {
-        const int32_t c = prm.coarse[st * prm.n_coarse + (prm.n_coarse == 1 ? 0 : m)];
-        cr = (int)(c & (N - 1));
-        const double d = (double)prm.fine_d[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
-        const double phi = (double)prm.fine_phi[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
-        dts = d / (double)N;                              // turns per channel of the fractional part
-        if (tid < 16) {
-            const int k = Plan::Q * tid;
-            const double t = -dts * (double)k - (double)((cr * k) & (N - 1)) / (double)N;
-            sph->step[tid] = phasor_turns(t);
-        } else if (tid == 16) {
-            double s, c_;
-            sincos(phi, &s, &c_);
-            sph->ephi = make_float2((float)c_, (float)s);
-            sincos(2.0 * phi, &s, &c_);
-            const float2 e2 = make_float2((float)c_, (float)s);
-            // exp(-i pi d_eff) = exp(-i pi d) * (-1)^cr
-            float2 h = phasor_turns(-0.5 * d);
-            if (cr & 1) { h.x = -h.x; h.y = -h.y; }
-            sph->c3 = cmulf(e2, h);
+    for (int pol = 0; pol < P; ++pol) {
+        const int64_t st = (int64_t)a * P + pol;
+        const float4 *grow = reinterpret_cast<const float4 *>(
+            prm.g + (((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * P + pol) * (int64_t)N);
+
+        // per-spectrum phasor set-up
+        double dts = 0.0;
+        int cr = 0;
+        if (prm.per_spectrum) {
+            const int32_t c = prm.coarse[st * prm.n_coarse + (prm.n_coarse == 1 ? 0 : m)];
+            cr = (int)(c & (N - 1));
+            const double d = (double)prm.fine_d[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
+            const double phi = (double)prm.fine_phi[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
+            dts = d / (double)N;                          // turns per channel of the fractional part
+            if (tid < 16) {
+                const int k = Plan::Q * tid;
+                const double t = -dts * (double)k - (double)((cr * k) & (N - 1)) / (double)N;
+                sph->step[tid] = phasor_turns(t);
+            } else if (tid == 16) {
+                double s, c_;
+                sincos(phi, &s, &c_);
+                sph->ephi = make_float2((float)c_, (float)s);
+                sincos(2.0 * phi, &s, &c_);
+                const float2 e2 = make_float2((float)c_, (float)s);
+                float2 h = phasor_turns(-0.5 * d);        // exp(-i pi d_eff) = exp(-i pi d) * (-1)^cr
+                if (cr & 1) { h.x = -h.x; h.y = -h.y; }
+                sph->c3 = cmulf(e2, h);
+            }
         }
-    }
 
-    fft_pass_first<Plan>(grow, sm, prm.tab.tw[0], tid);
-    __syncthreads();
-    fft_pass_mid<Plan, 2>(sm, prm.tab.tw[1], tid);
-    __syncthreads();
-    if constexpr (Plan::q == 4) {
-        fft_pass_mid<Plan, 3>(sm, prm.tab.tw[2], tid);
+        fft_pass_first<Plan>(grow, sm, prm.tab.tw[0], tid);
         __syncthreads();
+        fft_pass_mid<Plan, 2>(sm, prm.tab.tw[1], tid);
+        __syncthreads();
+        if constexpr (Plan::q == 4) {
+            fft_pass_mid<Plan, 3>(sm, prm.tab.tw[2], tid);
+            __syncthreads();
+        }
+        fft_pass_last<Plan, F32OUT>(sm, prm, a, pol, m, tid, stage, sph, dts, cr);
+        if (pol + 1 < P) __syncthreads();                 // exchange buffer and phasors are reused
     }
-    fft_pass_last<Plan, F32OUT>(sm, prm, a, pol, m, tid, stage, sph, dts, cr);
     if (!F32OUT) {
         __syncthreads();
         // coalesced copy-out of the staged record [n][P][2] int8

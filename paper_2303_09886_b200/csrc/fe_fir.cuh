@@ -5,7 +5,12 @@
 // A thread owns one 5-byte group = 4 consecutive *input* columns v0..v0+3 and walks down the rows
 // with a T-row sliding window of converted samples in registers and its 4*T weights in registers
 // (the paper's register sliding window), so every sample is loaded, unpacked and
-// converted exactly once per tile and every tap is one FMA lane-op.
+// converted exactly once per tile and every tap is one FMA lane-op (issued as packed FFMA2).
+//
+// Input staging.  Each warp owns a small ring of rows in shared memory (160 bytes per row: 32
+// lanes x 5 bytes) that it fills with 16-byte cp.async copies kDepth-1 rows ahead of use, so the
+// HBM/L2 latency is hidden without spending registers, and every global access is an aligned
+// 128-bit one (BASELINE.json north_star (a)).
 //
 // Coarse delay.  With c = N*cq + cr (0 <= cr < N), the sample that Eq. (1)
 // pairs with output column t of spectrum m and tap j is row m + j - cq - [t < cr], input column
@@ -14,7 +19,8 @@
 // row rotated by cr:  g'[v] = g[(v + cr) mod N].  The rotation is undone for free in the
 // frequency domain (circular shift theorem): X[k] = exp(-2 pi i k cr / N) * FFT(g')[k], which the
 // FFT epilogue folds into the fine-delay phasor.  Columns that wrap (v + cr >= N) read one row
-// earlier ("lag"); the single quad that straddles the wrap keeps the previous row's samples too.
+// earlier ("lag"): a thread whose four columns all lag reads the ring one slot behind; the single
+// quad that straddles the wrap (MIXED) reads both slots.
 //
 // Output: scratch rows g' in fp32, one row of N floats per (antenna, spectrum, pol); each group of
 // four columns is stored as (g0, g2, g1, g3) so that the FFT's first pass can load the packed
@@ -41,8 +47,19 @@ struct FirParams {
 };
 
 constexpr int kFirThreads = 128;
+constexpr int kFirWarps = kFirThreads / 32;
 constexpr int kFirColsPerThread = 4;
 constexpr int kFirColsPerBlock = kFirThreads * kFirColsPerThread;   // 512
+constexpr int kFirRowBytes = 160;                                   // per warp per row: 32 lanes x 5 bytes
+constexpr int kFirDepth = 8;                                        // ring slots per warp
+
+__device__ __forceinline__ void cp_async_16(uint32_t smem_addr, const void *gptr)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_addr), "l"(gptr) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N_PENDING>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N_PENDING) : "memory"); }
 
 // 5 bytes (big-endian bit stream) -> 4 sign-extended samples.  W0/W1 are the two little-endian
 // aligned words that contain the group; sel picks bytes b0..b3 as a big-endian word.
@@ -56,12 +73,17 @@ __device__ __forceinline__ void unpack_quad(uint32_t W0, uint32_t W1, uint32_t s
     s[3] = (float)((int32_t)(be2 << 22) >> 22);                 // bits  9..0
 }
 
-template <int T, int PF>
-__device__ __forceinline__ void fir_run(const FirParams &prm, const uint8_t *sbase, int64_t c, int64_t m0,
-                                        int n_out, int v0, float *grow0)
+// One run of n_out consecutive spectra with a constant coarse delay c, for this thread's quad.
+//   ring      this warp's shared-memory ring, kFirDepth slots of kFirRowBytes
+//   wsrc      global address of byte 0 of this warp's 160-byte segment in input row 0 of the stream
+template <int T, bool MIXED>
+__device__ __forceinline__ void fir_run(const FirParams &prm, const uint8_t *wsrc, unsigned char *ring, int64_t c,
+                                        int64_t m0, int n_out, int v0, float *grow0)
 {
-    static_assert(T % PF == 0, "prefetch depth must divide the tap count");
+    constexpr int D = kFirDepth;
+    static_assert(16 % D == 0 || D % 16 == 0, "ring depth must be compatible with the unroll");
     const int N = 1 << prm.lgN;
+    const int lane = threadIdx.x & 31;
     const int cr = (int)(c & (int64_t)(N - 1));
     const int64_t cq = (c - cr) >> prm.lgN;
 
@@ -82,77 +104,85 @@ __device__ __forceinline__ void fir_run(const FirParams &prm, const uint8_t *sba
             wB[j] = f2(__ldg(prm.weights + tc[1] + (size_t)N * j), __ldg(prm.weights + tc[3] + (size_t)N * j));
         }
     }
-    const bool mixed = lag[3] && !lag[0];
-    const int64_t base_row = m0 - cq - (lag[0] ? 1 : 0);        // input row of ring step 0
-    // valid ring steps: 0 <= base_row + rho < rows_in
-    const int64_t lo64 = -base_row, hi64 = prm.rows_in - base_row;
-    const int rho_lo = (int)max((int64_t)-1, min(lo64, (int64_t)0x3fffffff));
-    const int rho_hi = (int)max((int64_t)-1, min(hi64, (int64_t)0x3fffffff));
-
-    const int row_words = (N / 4 * 5) / 4;                      // row stride in 32-bit words
-    const int64_t byte0 = base_row * (int64_t)(N / 4 * 5) + (int64_t)(v0 / 4) * 5;
-    const uint32_t sh = (uint32_t)(byte0 & 3);
+    // Ring step rho of the warp holds input row  R0 + rho,  R0 = m0 - cq - 1.  A thread with no lag
+    // uses ring step rho+1 for its window step rho; a lagging thread uses ring step rho.
+    const int64_t R0 = m0 - cq - 1;
+    const int row_bytes = N / 4 * 5;
+    const uint32_t ring_s = (uint32_t)__cvta_generic_to_shared(ring);
+    const int rd_off = (lag[0] ? 0 : 1);                        // MIXED threads: lag[0] = false, lag[3] = true
+    const uint32_t sh = (uint32_t)((5 * lane) & 3);
     const uint32_t sel = (sh + 3) | ((sh + 2) << 4) | ((sh + 1) << 8) | (sh << 12);
-    const uint32_t *wp = reinterpret_cast<const uint32_t *>(sbase) + (byte0 >> 2);   // word of step 0
+    const uint32_t lane_word = (uint32_t)((5 * lane) >> 2) * 4u;          // byte offset of W0 inside a slot
 
-    auto fetch = [&](int rho, uint32_t &W0, uint32_t &W1) {
-        if (rho >= rho_lo && rho < rho_hi) {
-            const uint32_t *q = wp + (int64_t)rho * row_words;
-            W0 = __ldg(q);
-            W1 = __ldg(q + 1);
-        } else {
-            W0 = 0u;
-            W1 = 0u;
+    // valid ring steps: 0 <= R0 + rho < rows_in
+    const int64_t lo64 = -R0, hi64 = prm.rows_in - R0;
+    const int rho_lo = (int)max((int64_t)0, min(lo64, (int64_t)0x3fffffff));
+    const int rho_hi = (int)max((int64_t)0, min(hi64, (int64_t)0x3fffffff));
+    const uint8_t *src = wsrc + R0 * (int64_t)row_bytes + lane * 16;     // lanes 0..9 copy 16 bytes each
+
+    // issue the copy of ring step rho into slot rho % D (whole warp calls; lanes 0..9 act)
+    auto issue = [&](int rho, int slot) {
+        if (lane < 10) {
+            const uint32_t dst = ring_s + slot * kFirRowBytes + lane * 16;
+            if (rho >= rho_lo && rho < rho_hi)
+                cp_async_16(dst, src + (int64_t)rho * row_bytes);
+            else
+                asm volatile("st.shared.v4.u32 [%0], {%1,%1,%1,%1};" ::"r"(dst), "r"(0u) : "memory");
         }
+        cp_async_commit();
     };
-
-    float prev[4] = {0.f, 0.f, 0.f, 0.f};
-    if (mixed) {                                                // the quad that straddles the wrap
+    auto load_slot = [&](int slot, float (&s)[4]) {
         uint32_t W0, W1;
-        fetch(-1, W0, W1);
-        unpack_quad(W0, W1, sel, prev);
-    }
-
-    uint32_t raw0[PF], raw1[PF];
-#pragma unroll
-    for (int k = 0; k < PF; ++k) fetch(k, raw0[k], raw1[k]);
-
-    f2 rA[T], rB[T];                                            // sliding window, slot = rho mod T
-
-    auto insert = [&](int slot_pf, int rho, f2 &dstA, f2 &dstB) {
-        float s[4];
-        unpack_quad(raw0[slot_pf], raw1[slot_pf], sel, s);
-        fetch(rho + PF, raw0[slot_pf], raw1[slot_pf]);          // refill the prefetch slot
-        if (mixed) {
-            float t[4];
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                t[i] = lag[i] ? prev[i] : s[i];
-                prev[i] = s[i];
-            }
-            dstA = f2(t[0], t[2]);
-            dstB = f2(t[1], t[3]);
-        } else {
-            dstA = f2(s[0], s[2]);
-            dstB = f2(s[1], s[3]);
-        }
+        const uint32_t a = ring_s + slot * kFirRowBytes + lane_word;
+        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(W0) : "r"(a) : "memory");
+        asm volatile("ld.shared.u32 %0, [%1+4];" : "=r"(W1) : "r"(a) : "memory");
+        unpack_quad(W0, W1, sel, s);
     };
 
-    // warm-up: rows 0 .. T-2
+    // Protocol.  Ring step q (input row R0 + q) lives in slot q % D.  Window step w needs ring steps
+    // w (lagging columns) and w+1 (others).  Ring steps 0..D-1 are issued up front; at window step
+    // w >= 1, after the warp barrier, ring step w-1+D is issued into the slot ring step w-1 occupied
+    // (nobody needs it any more).  At the wait of window step w, D+w-1 groups have been committed and
+    // ring steps <= w+1 must be complete, so at most D-3 may be pending.
+    static_assert(D >= 4, "ring too shallow");
+    __syncwarp();                                               // previous run's reads of the ring are done
 #pragma unroll
-    for (int rho = 0; rho < T - 1; ++rho) insert(rho % PF, rho, rA[rho], rB[rho]);
+    for (int k = 0; k < D; ++k) issue(k, k);
+
+    f2 rA[T], rB[T];                                            // sliding window, slot = window step mod T
+
+    auto consume = [&](int w, int slot_cur, int slot_prev, int slot_refill, bool refill, f2 &dstA, f2 &dstB) {
+        cp_async_wait<D - 3>();
+        __syncwarp();                                           // copies visible; last step's reads finished
+        if (refill) issue(w - 1 + D, slot_refill);
+        float s[4];
+        if (MIXED) {
+            float sp[4];
+            load_slot(slot_cur, s);
+            load_slot(slot_prev, sp);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) s[i] = lag[i] ? sp[i] : s[i];
+        } else {
+            load_slot(rd_off ? slot_cur : slot_prev, s);
+        }
+        dstA = f2(s[0], s[2]);
+        dstB = f2(s[1], s[3]);
+    };
+
+    // warm-up: window steps 0 .. T-2
+#pragma unroll
+    for (int w = 0; w < T - 1; ++w) consume(w, (w + 1) % D, w % D, (w + D - 1) % D, w >= 1, rA[w % T], rB[w % T]);
 
     float4 *gp = reinterpret_cast<float4 *>(grow0 + v0);
     const size_t g_stride4 = ((size_t)N * prm.P) / 4;           // next spectrum, same pol (float4 units)
 
-    for (int i0 = 0; i0 < n_out; i0 += T) {
+    constexpr int U = (T % D == 0) ? T : (T * D);               // unroll so that both T and D indices are static
+    for (int i0 = 0; i0 < n_out; i0 += U) {
 #pragma unroll
-        for (int ii = 0; ii < T; ++ii) {
+        for (int ii = 0; ii < U; ++ii) {
             if (i0 + ii < n_out) {
-                constexpr int dummy = 0;
-                (void)dummy;
-                const int slot = (ii + T - 1) % T;
-                insert(slot % PF, i0 + ii + T - 1, rA[slot], rB[slot]);
+                const int w = ii + T - 1;                       // window step (mod U) inserted now
+                consume(i0 + w, (w + 1) % D, w % D, (w + D - 1) % D, true, rA[w % T], rB[w % T]);
                 f2 a0 = rA[ii % T] * wA[0], b0 = rB[ii % T] * wB[0];
                 f2 a1, b1;
                 if (T > 1) {
@@ -172,24 +202,27 @@ __device__ __forceinline__ void fir_run(const FirParams &prm, const uint8_t *sba
                     a0 = a0 + a1;
                     b0 = b0 + b1;
                 }
-                // (g0, g2, g1, g3)
-                stg_stream_f4(gp, make_float4(a0.v.x, a0.v.y, b0.v.x, b0.v.y));
+                stg_stream_f4(gp, make_float4(a0.v.x, a0.v.y, b0.v.x, b0.v.y));   // (g0, g2, g1, g3)
                 gp += g_stride4;
             }
         }
     }
+    cp_async_wait<0>();                                         // drain before the ring is reused
 }
 
-template <int T, int PF>
-__global__ void __launch_bounds__(kFirThreads) fir_kernel(const FirParams prm)
+template <int T>
+__global__ void __launch_bounds__(kFirThreads, 3) fir_kernel(const FirParams prm)
 {
+    __shared__ __align__(16) unsigned char ring_all[kFirWarps][kFirDepth * kFirRowBytes];
     const int N = 1 << prm.lgN;
     const int stream = blockIdx.z;
     const int a = stream / prm.P, p = stream - a * prm.P;
+    const int warp = threadIdx.x >> 5;
     const int v0 = (blockIdx.x * kFirThreads + threadIdx.x) * kFirColsPerThread;
     int64_t m = prm.m_begin + (int64_t)blockIdx.y * prm.rows_per_tile;
     const int64_t m_stop = min(m + (int64_t)prm.rows_per_tile, prm.m_end);
     const uint8_t *sbase = prm.in + (int64_t)stream * prm.stream_bytes;
+    const uint8_t *wsrc = sbase + (int64_t)(blockIdx.x * kFirWarps + warp) * kFirRowBytes;
     const int32_t *ctab = prm.coarse + (int64_t)stream * prm.n_coarse;
 
     while (m < m_stop) {
@@ -200,7 +233,15 @@ __global__ void __launch_bounds__(kFirThreads) fir_kernel(const FirParams prm)
             while (run_end < m_stop && ctab[run_end] == c) ++run_end;
         }
         float *grow0 = prm.g + (((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * prm.P + p) * (int64_t)N;
-        fir_run<T, PF>(prm, sbase, (int64_t)c, m, (int)(run_end - m), v0, grow0);
+        // does any quad of this warp straddle the wrap column N - cr ?  (warp-uniform decision)
+        const int cr = (int)((int64_t)c & (int64_t)(N - 1));
+        const int wv0 = v0 - (threadIdx.x & 31) * 4;            // first column of the warp
+        const int wrapcol = N - cr;                              // first lagging input column
+        const bool warp_mixed = (wrapcol & 3) != 0 && wrapcol > wv0 && wrapcol < wv0 + 128;
+        if (warp_mixed)
+            fir_run<T, true>(prm, wsrc, ring_all[warp], (int64_t)c, m, (int)(run_end - m), v0, grow0);
+        else
+            fir_run<T, false>(prm, wsrc, ring_all[warp], (int64_t)c, m, (int)(run_end - m), v0, grow0);
         m = run_end;
     }
 }

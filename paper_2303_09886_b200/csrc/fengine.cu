@@ -113,10 +113,12 @@ int launch_fft(fengine *fe, const FftParams &prm, int64_t chunk_len, cudaStream_
     static bool attr_set = false;
     if (!attr_set) {
         FE_CUDA(fe, cudaFuncSetAttribute(fft_kernel<Plan, F32OUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max));
+        FE_CUDA(fe, cudaFuncSetAttribute(fft_kernel<Plan, F32OUT>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                         (int)cudaSharedmemCarveoutMaxShared));
         attr_set = true;
     }
     dim3 grid((unsigned)chunk_len, (unsigned)fe->A);
-    fft_kernel<Plan, F32OUT><<<grid, Plan::tpf * fe->P, smem, stream>>>(prm);
+    fft_kernel<Plan, F32OUT><<<grid, Plan::tpf, smem, stream>>>(prm);
     return FENGINE_OK;
 }
 
@@ -137,10 +139,10 @@ int launch_fir(fengine *fe, const FirParams &prm, int64_t chunk_len, cudaStream_
     dim3 grid((unsigned)(fe->N / kFirColsPerBlock), (unsigned)((chunk_len + prm.rows_per_tile - 1) / prm.rows_per_tile),
               (unsigned)(fe->A * fe->P));
     switch (fe->T) {
-    case 2: fir_kernel<2, 2><<<grid, kFirThreads, 0, stream>>>(prm); break;
-    case 4: fir_kernel<4, 4><<<grid, kFirThreads, 0, stream>>>(prm); break;
-    case 8: fir_kernel<8, 4><<<grid, kFirThreads, 0, stream>>>(prm); break;
-    case 16: fir_kernel<16, 4><<<grid, kFirThreads, 0, stream>>>(prm); break;
+    case 2: fir_kernel<2><<<grid, kFirThreads, 0, stream>>>(prm); break;
+    case 4: fir_kernel<4><<<grid, kFirThreads, 0, stream>>>(prm); break;
+    case 8: fir_kernel<8><<<grid, kFirThreads, 0, stream>>>(prm); break;
+    case 16: fir_kernel<16><<<grid, kFirThreads, 0, stream>>>(prm); break;
     default: return fail(fe, FENGINE_ERR_INVALID_ARG, "no tiled FIR for T=%d", fe->T);
     }
     return FENGINE_OK;
