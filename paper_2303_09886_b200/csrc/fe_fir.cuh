@@ -76,26 +76,32 @@ __device__ __forceinline__ void unpack_quad(uint32_t W0, uint32_t W1, uint32_t s
 // One run of n_out consecutive spectra with a constant coarse delay c, for this thread's quad.
 //   ring      this warp's shared-memory ring, kFirDepth slots of kFirRowBytes
 //   wsrc      global address of byte 0 of this warp's 160-byte segment in input row 0 of the stream
-template <int T, bool MIXED>
-__device__ __forceinline__ void fir_run(const FirParams &prm, const uint8_t *wsrc, unsigned char *ring, int64_t c,
+//
+// Ring step q of the warp holds input row R0 + q, R0 = m0 - cq - 1, and every lane consumes the ring
+// steps in order, one per loop step, into its T-row register window.  After ring step q >= T-1 the
+// window holds rows R0+q-T+1 .. R0+q, which is spectrum q-T of the run for a column without lag and
+// spectrum q-T+1 for a lagging column: lagging columns simply run one spectrum ahead, so the inner
+// loop is identical for every lane and only the store row (and its bounds predicate) differs.
+template <int T>
+__device__ __forceinline__ void fir_run(const FirParams &prm, const uint8_t *wsrc, uint32_t ring_s, int64_t c,
                                         int64_t m0, int n_out, int v0, float *grow0)
 {
     constexpr int D = kFirDepth;
-    static_assert(16 % D == 0 || D % 16 == 0, "ring depth must be compatible with the unroll");
+    static_assert(D >= 4, "ring too shallow");
     const int N = 1 << prm.lgN;
     const int lane = threadIdx.x & 31;
     const int cr = (int)(c & (int64_t)(N - 1));
     const int64_t cq = (c - cr) >> prm.lgN;
 
     // output columns, lag flags and weights of this thread's four input columns
-    bool lag[4];
+    int lagi[4];
     f2 wA[T], wB[T];                                            // (col0, col2), (col1, col3)
     {
         int tc[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             const int t = v0 + i + cr;
-            lag[i] = t >= N;
+            lagi[i] = t >= N ? 1 : 0;
             tc[i] = t & (N - 1);
         }
 #pragma unroll
@@ -104,85 +110,75 @@ __device__ __forceinline__ void fir_run(const FirParams &prm, const uint8_t *wsr
             wB[j] = f2(__ldg(prm.weights + tc[1] + (size_t)N * j), __ldg(prm.weights + tc[3] + (size_t)N * j));
         }
     }
-    // Ring step rho of the warp holds input row  R0 + rho,  R0 = m0 - cq - 1.  A thread with no lag
-    // uses ring step rho+1 for its window step rho; a lagging thread uses ring step rho.
+    const int lag0 = lagi[0];
+    const bool mixed = lagi[3] != lagi[0];                      // the one quad that straddles the wrap column
     const int64_t R0 = m0 - cq - 1;
     const int row_bytes = N / 4 * 5;
-    const uint32_t ring_s = (uint32_t)__cvta_generic_to_shared(ring);
-    const int rd_off = (lag[0] ? 0 : 1);                        // MIXED threads: lag[0] = false, lag[3] = true
     const uint32_t sh = (uint32_t)((5 * lane) & 3);
     const uint32_t sel = (sh + 3) | ((sh + 2) << 4) | ((sh + 1) << 8) | (sh << 12);
-    const uint32_t lane_word = (uint32_t)((5 * lane) >> 2) * 4u;          // byte offset of W0 inside a slot
+    const uint32_t rd_addr = ring_s + (uint32_t)((5 * lane) >> 2) * 4u;     // W0 of this lane in slot 0
+    const uint32_t wr_addr = ring_s + (uint32_t)(lane < 10 ? lane : 0) * 16u;
+    const uint32_t is_copier = lane < 10 ? 1u : 0u;
 
-    // valid ring steps: 0 <= R0 + rho < rows_in
+    // valid ring steps: 0 <= R0 + q < rows_in
     const int64_t lo64 = -R0, hi64 = prm.rows_in - R0;
-    const int rho_lo = (int)max((int64_t)0, min(lo64, (int64_t)0x3fffffff));
-    const int rho_hi = (int)max((int64_t)0, min(hi64, (int64_t)0x3fffffff));
-    const uint8_t *src = wsrc + R0 * (int64_t)row_bytes + lane * 16;     // lanes 0..9 copy 16 bytes each
+    const int q_lo = (int)max((int64_t)0, min(lo64, (int64_t)0x3fffffff));
+    const int q_hi = (int)max((int64_t)0, min(hi64, (int64_t)0x3fffffff));
+    const uint8_t *src = wsrc + R0 * (int64_t)row_bytes + (lane < 10 ? lane : 0) * 16;   // ring step 0
 
-    // issue the copy of ring step rho into slot rho % D (whole warp calls; lanes 0..9 act)
-    auto issue = [&](int rho, int slot) {
-        if (lane < 10) {
-            const uint32_t dst = ring_s + slot * kFirRowBytes + lane * 16;
-            if (rho >= rho_lo && rho < rho_hi)
-                cp_async_16(dst, src + (int64_t)rho * row_bytes);
-            else
-                asm volatile("st.shared.v4.u32 [%0], {%1,%1,%1,%1};" ::"r"(dst), "r"(0u) : "memory");
-        }
-        cp_async_commit();
-    };
-    auto load_slot = [&](int slot, float (&s)[4]) {
-        uint32_t W0, W1;
-        const uint32_t a = ring_s + slot * kFirRowBytes + lane_word;
-        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(W0) : "r"(a) : "memory");
-        asm volatile("ld.shared.u32 %0, [%1+4];" : "=r"(W1) : "r"(a) : "memory");
-        unpack_quad(W0, W1, sel, s);
+    // copy ring step q into `slot` (lanes 0..9 move 16 bytes each; rows outside the batch are zero-filled)
+    auto issue = [&](int q, int slot) {
+        const uint32_t ok = (q >= q_lo && q < q_hi) ? is_copier : 0u;
+        const uint32_t zf = is_copier & ~ok;
+        asm volatile(
+            "{\n\t.reg .pred p, z;\n\t"
+            "setp.ne.u32 p, %2, 0;\n\t"
+            "setp.ne.u32 z, %3, 0;\n\t"
+            "@p cp.async.cg.shared.global [%0], [%1], 16;\n\t"
+            "@z st.shared.v4.u32 [%0], {%4, %4, %4, %4};\n\t"
+            "cp.async.commit_group;\n\t}"
+            ::"r"(wr_addr + slot * kFirRowBytes), "l"(src), "r"(ok), "r"(zf), "r"(0u) : "memory");
+        src += row_bytes;
     };
 
-    // Protocol.  Ring step q (input row R0 + q) lives in slot q % D.  Window step w needs ring steps
-    // w (lagging columns) and w+1 (others).  Ring steps 0..D-1 are issued up front; at window step
-    // w >= 1, after the warp barrier, ring step w-1+D is issued into the slot ring step w-1 occupied
-    // (nobody needs it any more).  At the wait of window step w, D+w-1 groups have been committed and
-    // ring steps <= w+1 must be complete, so at most D-3 may be pending.
-    static_assert(D >= 4, "ring too shallow");
     __syncwarp();                                               // previous run's reads of the ring are done
 #pragma unroll
     for (int k = 0; k < D; ++k) issue(k, k);
 
-    f2 rA[T], rB[T];                                            // sliding window, slot = window step mod T
+    f2 rA[T], rB[T];                                            // sliding window, slot = ring step mod T
 
-    auto consume = [&](int w, int slot_cur, int slot_prev, int slot_refill, bool refill, f2 &dstA, f2 &dstB) {
-        cp_async_wait<D - 3>();
+    // Protocol: ring steps 0..D-1 are issued up front; at loop step q >= 1, after the warp barrier,
+    // ring step q-1+D is issued into the slot ring step q-1 occupied.  At the wait of step q, D+q-1
+    // groups have been committed and ring steps <= q must be complete: at most D-2 may be pending.
+    auto consume = [&](int q, int slot, int slot_refill, bool refill, f2 &dstA, f2 &dstB) {
+        cp_async_wait<D - 2>();
         __syncwarp();                                           // copies visible; last step's reads finished
-        if (refill) issue(w - 1 + D, slot_refill);
+        if (refill) issue(q - 1 + D, slot_refill);
+        uint32_t W0, W1;
+        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(W0) : "r"(rd_addr + slot * kFirRowBytes) : "memory");
+        asm volatile("ld.shared.u32 %0, [%1+4];" : "=r"(W1) : "r"(rd_addr + slot * kFirRowBytes) : "memory");
         float s[4];
-        if (MIXED) {
-            float sp[4];
-            load_slot(slot_cur, s);
-            load_slot(slot_prev, sp);
-#pragma unroll
-            for (int i = 0; i < 4; ++i) s[i] = lag[i] ? sp[i] : s[i];
-        } else {
-            load_slot(rd_off ? slot_cur : slot_prev, s);
-        }
+        unpack_quad(W0, W1, sel, s);
         dstA = f2(s[0], s[2]);
         dstB = f2(s[1], s[3]);
     };
 
-    // warm-up: window steps 0 .. T-2
+    // warm-up: ring steps 0 .. T-2
 #pragma unroll
-    for (int w = 0; w < T - 1; ++w) consume(w, (w + 1) % D, w % D, (w + D - 1) % D, w >= 1, rA[w % T], rB[w % T]);
+    for (int q = 0; q < T - 1; ++q) consume(q, q % D, (q + D - 1) % D, q >= 1, rA[q % T], rB[q % T]);
 
-    float4 *gp = reinterpret_cast<float4 *>(grow0 + v0);
-    const size_t g_stride4 = ((size_t)N * prm.P) / 4;           // next spectrum, same pol (float4 units)
+    // loop step i (0-based) consumes ring step i + T - 1 and completes spectrum  i - 1 + lag  of the run
+    const size_t g_stride = (size_t)N * prm.P;                  // next spectrum, same pol (floats)
+    float *gp = grow0 + v0 + ((int64_t)lag0 - 1) * (int64_t)g_stride;
+    const int n_steps = n_out + 1;
 
     constexpr int U = (T % D == 0) ? T : (T * D);               // unroll so that both T and D indices are static
-    for (int i0 = 0; i0 < n_out; i0 += U) {
+    for (int i0 = 0; i0 < n_steps; i0 += U) {
 #pragma unroll
         for (int ii = 0; ii < U; ++ii) {
-            if (i0 + ii < n_out) {
-                const int w = ii + T - 1;                       // window step (mod U) inserted now
-                consume(i0 + w, (w + 1) % D, w % D, (w + D - 1) % D, true, rA[w % T], rB[w % T]);
+            if (i0 + ii < n_steps) {
+                const int q = ii + T - 1;                       // ring step (mod U) consumed now
+                consume(i0 + q, q % D, (q + D - 1) % D, true, rA[q % T], rB[q % T]);
                 f2 a0 = rA[ii % T] * wA[0], b0 = rB[ii % T] * wB[0];
                 f2 a1, b1;
                 if (T > 1) {
@@ -202,8 +198,20 @@ __device__ __forceinline__ void fir_run(const FirParams &prm, const uint8_t *wsr
                     a0 = a0 + a1;
                     b0 = b0 + b1;
                 }
-                stg_stream_f4(gp, make_float4(a0.v.x, a0.v.y, b0.v.x, b0.v.y));   // (g0, g2, g1, g3)
-                gp += g_stride4;
+                const int spec = i0 + ii - 1 + lag0;            // spectrum of the run this window completes
+                if (!mixed) {
+                    if (spec >= 0 && spec < n_out)
+                        stg_stream_f4(reinterpret_cast<float4 *>(gp), make_float4(a0.v.x, a0.v.y, b0.v.x, b0.v.y));
+                } else {                                        // columns of this quad belong to two spectra
+                    const float gv[4] = {a0.v.x, b0.v.x, a0.v.y, b0.v.y};          // g0, g1, g2, g3
+                    const int pos[4] = {0, 2, 1, 3};                                  // stored as (g0, g2, g1, g3)
+#pragma unroll
+                    for (int cidx = 0; cidx < 4; ++cidx) {
+                        const int sp = i0 + ii - 1 + lagi[cidx];
+                        if (sp >= 0 && sp < n_out) gp[(int64_t)(lagi[cidx] - lag0) * (int64_t)g_stride + pos[cidx]] = gv[cidx];
+                    }
+                }
+                gp += g_stride;
             }
         }
     }
@@ -224,6 +232,7 @@ __global__ void __launch_bounds__(kFirThreads, 3) fir_kernel(const FirParams prm
     const uint8_t *sbase = prm.in + (int64_t)stream * prm.stream_bytes;
     const uint8_t *wsrc = sbase + (int64_t)(blockIdx.x * kFirWarps + warp) * kFirRowBytes;
     const int32_t *ctab = prm.coarse + (int64_t)stream * prm.n_coarse;
+    const uint32_t ring_s = (uint32_t)__cvta_generic_to_shared(ring_all[warp]);
 
     while (m < m_stop) {
         const int32_t c = ctab[prm.n_coarse == 1 ? 0 : m];
@@ -233,15 +242,7 @@ __global__ void __launch_bounds__(kFirThreads, 3) fir_kernel(const FirParams prm
             while (run_end < m_stop && ctab[run_end] == c) ++run_end;
         }
         float *grow0 = prm.g + (((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * prm.P + p) * (int64_t)N;
-        // does any quad of this warp straddle the wrap column N - cr ?  (warp-uniform decision)
-        const int cr = (int)((int64_t)c & (int64_t)(N - 1));
-        const int wv0 = v0 - (threadIdx.x & 31) * 4;            // first column of the warp
-        const int wrapcol = N - cr;                              // first lagging input column
-        const bool warp_mixed = (wrapcol & 3) != 0 && wrapcol > wv0 && wrapcol < wv0 + 128;
-        if (warp_mixed)
-            fir_run<T, true>(prm, wsrc, ring_all[warp], (int64_t)c, m, (int)(run_end - m), v0, grow0);
-        else
-            fir_run<T, false>(prm, wsrc, ring_all[warp], (int64_t)c, m, (int)(run_end - m), v0, grow0);
+        fir_run<T>(prm, wsrc, ring_s, (int64_t)c, m, (int)(run_end - m), v0, grow0);
         m = run_end;
     }
 }
