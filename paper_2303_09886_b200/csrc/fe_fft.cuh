@@ -101,18 +101,25 @@ struct Dif {
 // ------------------------------------------------------------------------------------------------
 // FFT plan (compile time)
 // ------------------------------------------------------------------------------------------------
-template <int N_CH, int NPASS, int R1, int R2, int R3, int R4, int TPF>
+template <int N_CH, int NPASS, int R1, int R2, int R3, int R4, int TPF, int SWEEPS = 1>
 struct FftPlan {
     static constexpr int n = N_CH;
     static constexpr int q = NPASS;
     static constexpr int tpf = TPF;                       // threads per pol-FFT
+    // SWEEPS = 2 (n = 32768, whose 256 KiB working set exceeds one SM's shared memory): the first
+    // pass is a radix-R1 butterfly of which sweep h keeps only the outputs k1 = h (mod 2), i.e. the
+    // top radix-2 stage of the decimation in frequency splits the transform into two independent
+    // n/2-point halves (even / odd channels) that go through the exchange buffer one after the other.
+    static constexpr int sweeps = SWEEPS;
+    static_assert(SWEEPS == 1 || SWEEPS == 2, "1 or 2 sweeps");
+    static_assert(SWEEPS == 1 || R1 % 2 == 0, "two sweeps need an even first radix");
     static_assert(NPASS == 3 || NPASS == 4, "3 or 4 passes");
     static_assert(R1 * R2 * R3 * R4 == N_CH, "radices must multiply to n");
     static_assert(NPASS == 4 || R4 == 1, "R4 unused with 3 passes");
     __host__ __device__ static constexpr int radix(int p) { return p == 1 ? R1 : p == 2 ? R2 : p == 3 ? R3 : R4; }
     static constexpr int Rq = NPASS == 3 ? R3 : R4;
     static constexpr int Q = N_CH / Rq;                   // residues handled by the last pass
-    static constexpr int units = N_CH / 2;                // 16-byte units per pol-FFT
+    static constexpr int units = N_CH / 2 / SWEEPS;       // 16-byte units in the exchange buffer
     // M_p = R_{p+1} * ... * R_q  (M_0 = n)
     __host__ __device__ static constexpr int M(int p)
     {
@@ -182,6 +189,50 @@ __device__ __forceinline__ void fft_pass_first(const float4 *__restrict__ grow, 
     }
 }
 
+// top radix-2 stage of a two-sweep first pass, element J (compile-time recursion so that W_R1^J is constant)
+template <class Plan, int H, int J>
+__device__ __forceinline__ void sweep_half(const float4 *__restrict__ grow, int col, cx<f2> (&a)[Plan::radix(1) / 2])
+{
+    constexpr int R = Plan::radix(1), RH = R / 2;
+    constexpr int ncol = Plan::S(1);
+    if constexpr (J < RH) {
+        const float4 u = ldg_stream_f4(grow + J * ncol + col);
+        const float4 v = ldg_stream_f4(grow + (J + RH) * ncol + col);
+        const cx<f2> xu = {f2(u.x, u.y), f2(u.z, u.w)}, xv = {f2(v.x, v.y), f2(v.z, v.w)};
+        if constexpr (H == 0)
+            a[J] = cadd(xu, xv);
+        else
+            a[J] = mul_w<R, J, f2>(csub(xu, xv));
+        sweep_half<Plan, H, J + 1>(grow, col, a);
+    }
+}
+
+// ---- pass 1 of a two-sweep plan: sweep H keeps the outputs k1 = 2 k'' + H of the radix-R1 butterfly.
+// Its top radix-2 stage is a[j] = x[j] + x[j + R1/2] (H = 0) or (x[j] - x[j + R1/2]) W_R1^j (H = 1);
+// the radix-R1/2 butterfly of a then gives k'' in natural order.  The row is read once per sweep.
+template <class Plan, int H>
+__device__ __forceinline__ void fft_pass_first_sweep(const float4 *__restrict__ grow, float4 *sm,
+                                                     const float4 *__restrict__ tw, int tid)
+{
+    constexpr int R = Plan::radix(1), RH = R / 2;
+    constexpr int ncol = Plan::S(1);
+    for (int col = tid; col < ncol; col += Plan::tpf) {
+        cx<f2> a[RH];
+        sweep_half<Plan, H, 0>(grow, col, a);
+        Dif<RH, f2>::run(a);
+#pragma unroll
+        for (int kk = 0; kk < RH; ++kk) {
+            const int k1 = 2 * kk + H;
+            cx<f2> y = a[kk];
+            if (k1 > 0) {
+                const float4 w = __ldg(tw + k1 * ncol + col);
+                y = cmul(a[kk], f2(w.x, w.y), f2(w.z, w.w));
+            }
+            sm[swz<Plan>(kk * ncol + col)] = make_float4(y.re.v.x, y.re.v.y, y.im.v.x, y.im.v.y);
+        }
+    }
+}
+
 // ---- middle pass p: shared -> butterfly -> twiddle -> shared (in place) -----------------------------
 template <class Plan, int PASS>
 __device__ __forceinline__ void fft_pass_mid(float4 *sm, const float4 *__restrict__ tw, int tid)
@@ -220,8 +271,9 @@ __device__ __forceinline__ int residue_to_store(int K)
 #pragma unroll
     for (int p = 1; p < Plan::q; ++p) {
         const int r = Plan::radix(p);
-        const int d = rem % r;
+        int d = rem % r;
         rem /= r;
+        if (p == 1) d /= Plan::sweeps;                    // two sweeps: the buffer holds k1 = 2 d + h
         store = store * r + d;
     }
     return store;
@@ -272,7 +324,7 @@ struct SpectrumPhase {       // shared, per pol: filled once per spectrum in per
 template <class Plan, bool F32OUT>
 __device__ __forceinline__ void fft_pass_last(const float4 *sm, const FftParams &prm, int a, int pol, int64_t m,
                                               int tid, uint16_t *stage, const SpectrumPhase *sph,
-                                              double d_eff_turn_scale, int cr)
+                                              double d_eff_turn_scale, int cr, int sweep)
 {
     constexpr int Rq = Plan::Rq, Q = Plan::Q, n = Plan::n, N = 2 * n;
     const float2 *__restrict__ tpost = prm.tab.tpost;
@@ -281,7 +333,9 @@ __device__ __forceinline__ void fft_pass_last(const float4 *sm, const FftParams 
     float *yout = nullptr;
     if (F32OUT) yout = prm.out_f32 + (((int64_t)a * prm.n_spectra + m) * n) * prm.P * 2 + pol * 2;
 
-    for (int pidx = tid; pidx < Q / 2; pidx += Plan::tpf) {
+    constexpr int SW = Plan::sweeps;
+    for (int jdx = tid; jdx < Q / 2 / SW; jdx += Plan::tpf) {
+        const int pidx = SW * jdx + sweep;                // residue K of this sweep's parity
         cx<float> zA[Rq], zB[Rq];
         const bool special = pidx == 0;
         fft_load_residue<Plan>(sm, pidx, zA);
@@ -346,8 +400,8 @@ __device__ __forceinline__ void fft_pass_last(const float4 *sm, const FftParams 
                 *reinterpret_cast<float2 *>(yout + (int64_t)kA * prm.P * 2) = make_float2(yAr, yAi);
                 if (kB < n) *reinterpret_cast<float2 *>(yout + (int64_t)kB * prm.P * 2) = make_float2(yBr, yBi);
             } else {
-                stage[kA * prm.P + pol] = (uint16_t)quantize_pair(yAr, yAi);
-                if (kB < n) stage[kB * prm.P + pol] = (uint16_t)quantize_pair(yBr, yBi);
+                stage[(kA / SW) * prm.P + pol] = (uint16_t)quantize_pair(yAr, yAi);
+                if (kB < n) stage[(kB / SW) * prm.P + pol] = (uint16_t)quantize_pair(yBr, yBi);
             }
         }
         if (special) {                                    // channel n/2: X = conj Z[n/2]
@@ -364,7 +418,7 @@ __device__ __forceinline__ void fft_pass_last(const float4 *sm, const FftParams 
             if (F32OUT)
                 *reinterpret_cast<float2 *>(yout + (int64_t)(n / 2) * prm.P * 2) = make_float2(yr, yi);
             else
-                stage[(n / 2) * prm.P + pol] = (uint16_t)quantize_pair(yr, yi);
+                stage[(n / 2 / SW) * prm.P + pol] = (uint16_t)quantize_pair(yr, yi);
         }
     }
 }
@@ -372,74 +426,98 @@ __device__ __forceinline__ void fft_pass_last(const float4 *sm, const FftParams 
 template <class Plan>
 constexpr size_t fft_smem_bytes(int P)
 {
-    return (size_t)Plan::units * 16 + (size_t)Plan::n * P * 2 + sizeof(SpectrumPhase);
+    return (size_t)Plan::units * 16 + (size_t)(Plan::n / Plan::sweeps) * P * 2 + sizeof(SpectrumPhase);
 }
 
 // One CTA per (antenna, spectrum); the pols are transformed one after the other through the same
-// exchange buffer (small CTAs, several per SM, each at a different phase of its spectrum).
+// exchange buffer (small CTAs, several per SM, each at a different phase of its spectrum).  A
+// two-sweep plan (n = 32768) runs the whole sequence once for the even and once for the odd channels.
 template <class Plan, bool F32OUT>
-__global__ void __launch_bounds__(Plan::tpf, 512 / Plan::tpf) fft_kernel(const FftParams prm)
+__global__ void __launch_bounds__(Plan::tpf, (512 / Plan::tpf) > 0 ? (512 / Plan::tpf) : 1) fft_kernel(const FftParams prm)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    constexpr int n = Plan::n, N = 2 * n;
+    constexpr int n = Plan::n, N = 2 * n, SW = Plan::sweeps;
     const int P = prm.P;
     float4 *sm = reinterpret_cast<float4 *>(smem_raw);
     uint16_t *stage = reinterpret_cast<uint16_t *>(smem_raw + (size_t)Plan::units * 16);
-    SpectrumPhase *sph = reinterpret_cast<SpectrumPhase *>(smem_raw + (size_t)Plan::units * 16 + (size_t)n * P * 2);
+    SpectrumPhase *sph = reinterpret_cast<SpectrumPhase *>(smem_raw + (size_t)Plan::units * 16 + (size_t)(n / SW) * P * 2);
 
     const int tid = threadIdx.x;
     const int a = blockIdx.y;
     const int64_t m = prm.m_begin + blockIdx.x;
     if (m >= prm.m_end) return;
 
-    for (int pol = 0; pol < P; ++pol) {
-        const int64_t st = (int64_t)a * P + pol;
-        const float4 *grow = reinterpret_cast<const float4 *>(
-            prm.g + (((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * P + pol) * (int64_t)N);
+    for (int sweep = 0; sweep < SW; ++sweep) {
+        for (int pol = 0; pol < P; ++pol) {
+            const int64_t st = (int64_t)a * P + pol;
+            const float4 *grow = reinterpret_cast<const float4 *>(
+                prm.g + (((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * P + pol) * (int64_t)N);
 
-        // per-spectrum phasor set-up
-        double dts = 0.0;
-        int cr = 0;
-        if (prm.per_spectrum) {
-            const int32_t c = prm.coarse[st * prm.n_coarse + (prm.n_coarse == 1 ? 0 : m)];
-            cr = (int)(c & (N - 1));
-            const double d = (double)prm.fine_d[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
-            const double phi = (double)prm.fine_phi[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
-            dts = d / (double)N;                          // turns per channel of the fractional part
-            if (tid < 16) {
-                const int k = Plan::Q * tid;
-                const double t = -dts * (double)k - (double)((cr * k) & (N - 1)) / (double)N;
-                sph->step[tid] = phasor_turns(t);
-            } else if (tid == 16) {
-                double s, c_;
-                sincos(phi, &s, &c_);
-                sph->ephi = make_float2((float)c_, (float)s);
-                sincos(2.0 * phi, &s, &c_);
-                const float2 e2 = make_float2((float)c_, (float)s);
-                float2 h = phasor_turns(-0.5 * d);        // exp(-i pi d_eff) = exp(-i pi d) * (-1)^cr
-                if (cr & 1) { h.x = -h.x; h.y = -h.y; }
-                sph->c3 = cmulf(e2, h);
+            // per-spectrum phasor set-up
+            double dts = 0.0;
+            int cr = 0;
+            if (prm.per_spectrum) {
+                const int32_t c = prm.coarse[st * prm.n_coarse + (prm.n_coarse == 1 ? 0 : m)];
+                cr = (int)(c & (N - 1));
+                const double d = (double)prm.fine_d[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
+                const double phi = (double)prm.fine_phi[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
+                dts = d / (double)N;                      // turns per channel of the fractional part
+                if (tid < 16) {
+                    const int k = Plan::Q * tid;
+                    const double t = -dts * (double)k - (double)((cr * k) & (N - 1)) / (double)N;
+                    sph->step[tid] = phasor_turns(t);
+                } else if (tid == 16) {
+                    double s, c_;
+                    sincos(phi, &s, &c_);
+                    sph->ephi = make_float2((float)c_, (float)s);
+                    sincos(2.0 * phi, &s, &c_);
+                    const float2 e2 = make_float2((float)c_, (float)s);
+                    float2 h = phasor_turns(-0.5 * d);    // exp(-i pi d_eff) = exp(-i pi d) * (-1)^cr
+                    if (cr & 1) { h.x = -h.x; h.y = -h.y; }
+                    sph->c3 = cmulf(e2, h);
+                }
+            }
+
+            if constexpr (SW == 1) {
+                fft_pass_first<Plan>(grow, sm, prm.tab.tw[0], tid);
+            } else {
+                if (sweep == 0)
+                    fft_pass_first_sweep<Plan, 0>(grow, sm, prm.tab.tw[0], tid);
+                else
+                    fft_pass_first_sweep<Plan, 1>(grow, sm, prm.tab.tw[0], tid);
+            }
+            __syncthreads();
+            fft_pass_mid<Plan, 2>(sm, prm.tab.tw[1], tid);
+            __syncthreads();
+            if constexpr (Plan::q == 4) {
+                fft_pass_mid<Plan, 3>(sm, prm.tab.tw[2], tid);
+                __syncthreads();
+            }
+            fft_pass_last<Plan, F32OUT>(sm, prm, a, pol, m, tid, stage, sph, dts, cr, sweep);
+            if (pol + 1 < P || sweep + 1 < SW) __syncthreads();   // exchange buffer and phasors are reused
+        }
+        if (!F32OUT) {
+            __syncthreads();
+            int8_t *rec = prm.out + (((int64_t)a * prm.n_spectra + m) * n) * P * 2;
+            if constexpr (SW == 1) {
+                // coalesced copy-out of the staged record [n][P][2] int8
+                const int n_vec = n * P * 2 / 16;
+                uint4 *dst = reinterpret_cast<uint4 *>(rec);
+                const uint4 *src = reinterpret_cast<const uint4 *>(stage);
+                for (int i = threadIdx.x; i < n_vec; i += blockDim.x) stg_stream_u4(dst + i, src[i]);
+            } else {
+                // the stage holds the channels k = SW i + sweep: [n / SW][P][2] int8, one P*2-byte group each
+                if (P == 2) {
+                    const uint32_t *src = reinterpret_cast<const uint32_t *>(stage);
+                    uint32_t *dst = reinterpret_cast<uint32_t *>(rec);
+                    for (int i = threadIdx.x; i < n / SW; i += blockDim.x) dst[SW * i + sweep] = src[i];
+                } else {
+                    uint16_t *dst = reinterpret_cast<uint16_t *>(rec);
+                    for (int i = threadIdx.x; i < n / SW; i += blockDim.x) dst[SW * i + sweep] = stage[i];
+                }
+                if (sweep + 1 < SW) __syncthreads();      // stage is reused by the next sweep
             }
         }
-
-        fft_pass_first<Plan>(grow, sm, prm.tab.tw[0], tid);
-        __syncthreads();
-        fft_pass_mid<Plan, 2>(sm, prm.tab.tw[1], tid);
-        __syncthreads();
-        if constexpr (Plan::q == 4) {
-            fft_pass_mid<Plan, 3>(sm, prm.tab.tw[2], tid);
-            __syncthreads();
-        }
-        fft_pass_last<Plan, F32OUT>(sm, prm, a, pol, m, tid, stage, sph, dts, cr);
-        if (pol + 1 < P) __syncthreads();                 // exchange buffer and phasors are reused
-    }
-    if (!F32OUT) {
-        __syncthreads();
-        // coalesced copy-out of the staged record [n][P][2] int8
-        const int n_vec = n * P * 2 / 16;
-        uint4 *dst = reinterpret_cast<uint4 *>(prm.out + (((int64_t)a * prm.n_spectra + m) * n) * P * 2);
-        const uint4 *src = reinterpret_cast<const uint4 *>(stage);
-        for (int i = threadIdx.x; i < n_vec; i += blockDim.x) stg_stream_u4(dst + i, src[i]);
     }
 }
 

@@ -87,8 +87,10 @@ using Plan1024 = FftPlan<1024, 3, 8, 8, 16, 1, 64>;
 using Plan2048 = FftPlan<2048, 3, 8, 16, 16, 1, 64>;
 using Plan4096 = FftPlan<4096, 3, 16, 16, 16, 1, 128>;
 using Plan8192 = FftPlan<8192, 4, 8, 8, 8, 16, 256>;
+using Plan16384 = FftPlan<16384, 4, 16, 16, 8, 8, 512>;
+using Plan32768 = FftPlan<32768, 4, 32, 16, 8, 8, 512, 2>;     // two sweeps of 16384 points (fe_fft.cuh)
 
-bool tiled_n(int n) { return n == 1024 || n == 2048 || n == 4096 || n == 8192; }
+bool tiled_n(int n) { return n >= 1024 && n <= 32768; }
 bool tiled_T(int T) { return T == 2 || T == 4 || T == 8 || T == 16; }
 
 template <class Plan>
@@ -130,6 +132,8 @@ int launch_fft_n(fengine *fe, const FftParams &prm, int64_t chunk_len, cudaStrea
     case 2048: return launch_fft<Plan2048, F32OUT>(fe, prm, chunk_len, stream);
     case 4096: return launch_fft<Plan4096, F32OUT>(fe, prm, chunk_len, stream);
     case 8192: return launch_fft<Plan8192, F32OUT>(fe, prm, chunk_len, stream);
+    case 16384: return launch_fft<Plan16384, F32OUT>(fe, prm, chunk_len, stream);
+    case 32768: return launch_fft<Plan32768, F32OUT>(fe, prm, chunk_len, stream);
     }
     return fail(fe, FENGINE_ERR_INVALID_ARG, "no tiled FFT plan for n=%d", fe->n);
 }
@@ -350,6 +354,8 @@ fengine_t *fengine_create_batched(int n_antennas, int n_channels, int taps, int 
         case 2048: rc = build_tables<Plan2048>(fe); break;
         case 4096: rc = build_tables<Plan4096>(fe); break;
         case 8192: rc = build_tables<Plan8192>(fe); break;
+        case 16384: rc = build_tables<Plan16384>(fe); break;
+        case 32768: rc = build_tables<Plan32768>(fe); break;
         }
         ok = rc == FENGINE_OK;
     }

@@ -188,6 +188,12 @@ def test_config1_full(torch, fb):
     (4, dict(n_spectra=130, n_antennas=1, sigma=182.0)),
     (5, dict(n_spectra=40, n_antennas=3, n_channels=1024)),
     (5, dict(n_spectra=33, n_antennas=2, n_channels=8192)),
+    (3, dict(n_spectra=9, n_antennas=2)),                       # n = 32768: two-sweep FFT
+    (3, dict(n_spectra=1, n_antennas=1)),
+    (5, dict(n_spectra=11, n_antennas=2, n_channels=32768)),
+    (5, dict(n_spectra=19, n_antennas=2, n_channels=16384)),
+    (4, dict(n_spectra=70, n_antennas=1, n_channels=32768)),    # per-spectrum delay tables at n = 32768
+    (4, dict(n_spectra=70, n_antennas=1, n_channels=16384)),
 ])
 def test_configs_reduced(torch, fb, cfg, kw):
     w = si.make_workload(cfg, **kw)
@@ -209,6 +215,9 @@ def test_configs_reduced(torch, fb, cfg, kw):
     (2048, 4, 65, 1, 2, False, (5, 6)),
     (4096, 2, 66, 1, 2, False, (8190, 8191)),
     (4096, 16, 129, 1, 2, False, (-1, 0)),
+    (16384, 4, 5, 1, 1, True, (-40000, 40000)),     # one pol, per-spectrum random delays beyond a row
+    (32768, 2, 3, 1, 1, False, (65535, 65536)),     # one pol, largest sub-row delay
+    (32768, 8, 4, 2, 2, True, (-70000, 140000)),
 ])
 def test_shapes_and_edges(torch, fb, n, T, S, A, P, per_spectrum, crange):
     w = si.custom_workload(A=A, n=n, T=T, S=S, P=P, seed=25, per_spectrum=per_spectrum, random_weights=(n <= 64),
@@ -302,6 +311,56 @@ def test_argument_errors(torch, fb):
 # ----------------------------------------------------------------------------------------------
 # full size, in the launch configuration bench.py times: sampled spectra against the oracle
 # ----------------------------------------------------------------------------------------------
+def _full_size_sampled(torch, fb, w, label, n_random=8, direct=3):
+    """Run the whole batch on the GPU; compare sampled spectra (first / last / random) with the oracle."""
+    fe = make_engine(fb, w)
+    d_in = torch.from_numpy(w.packed.reshape(-1)).cuda()
+    d_out = torch.zeros(fe.output_shape(w.S), dtype=torch.int8, device="cuda")
+    fe.process(d_in, d_out, w.S)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(7)
+    sel = np.unique(np.concatenate([[0, 1, 15, 16, 63, 64, 65, w.S - 2, w.S - 1], rng.integers(0, w.S, n_random)]))
+    sel = sel[(sel >= 0) & (sel < w.S)]
+    idx = torch.from_numpy(sel).cuda()
+    got = {"out": d_out[:, idx].cpu().numpy()}
+    assert int(d_out.min()) >= -127 and int(d_out.max()) <= 127
+    assert float(torch.count_nonzero(d_out)) / d_out.numel() > 0.8      # nothing left unwritten
+    del d_out
+    # pre-quantisation values of the sampled spectra: rerun them as a short batch is not possible
+    # (different windows), so take them from a float run of the whole batch, freed right after
+    d_y = torch.zeros(fe.output_shape(w.S), dtype=torch.float32, device="cuda")
+    fe.process_f32(d_in, d_y, w.S)
+    torch.cuda.synchronize()
+    y = d_y[:, idx].cpu().numpy().astype(np.float64)
+    got["Y"] = y[..., 0] + 1j * y[..., 1]
+    per = w.coarse.shape[2] > 1
+    for _ in range(direct):                                     # one-by-one definition check (NT-term DTFT)
+        a, p = int(rng.integers(w.A)), int(rng.integers(2))
+        m, k = int(rng.integers(w.S)), int(rng.integers(w.n))
+        yref = oracle.direct_channel(w.packed[a, p], w.L, w.n, w.T, w.weights, m, int(w.coarse[a, p, m if per else 0]),
+                                     w.fine_delay[a, p, m if per else 0], w.phase[a, p, m if per else 0],
+                                     w.gains[a, p, k], k)
+        yg = d_y[a, m, k, p].cpu().numpy().astype(np.float64)
+        rms = float(np.sqrt(np.mean(np.abs(got["Y"][a, :, :, p]) ** 2)))
+        assert abs(complex(yg[0], yg[1]) - yref) < 2e-4 * rms, (a, p, m, k)
+    del d_y
+    ref = oracle_run(w, sel=sel)
+    worst = check_parity(got, ref, label)
+    print(f"{label}: worst err/RMS over {len(sel)} sampled spectra = {worst:.3e}")
+
+
+def test_config3_full_size_sampled(torch, fb):
+    w = si.make_workload(3)                                      # 4 antennas x 2 pols, n=32768, 2^26 samples per pol
+    assert w.S == 1009
+    _full_size_sampled(torch, fb, w, "config3 full size", n_random=4)
+
+
+def test_config4_full_size_sampled(torch, fb):
+    w = si.make_workload(4)                                      # 8 antennas, n=8192, per-spectrum delay tables
+    assert w.S == 2033
+    _full_size_sampled(torch, fb, w, "config4 full size", n_random=6)
+
+
 def test_config2_full_size_sampled(torch, fb):
     w = si.make_workload(2)                                      # 4 antennas x 2 pols, n=4096, 2^24 samples per pol
     assert w.S == 2033
