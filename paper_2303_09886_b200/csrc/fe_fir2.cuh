@@ -1,0 +1,203 @@
+// fe_fir2.cuh -- steps 1-3 of the path for the pol-packed layout: unpack + coarse delay + polyphase
+// FIR (Eq. (1)) of BOTH polarisations of an antenna in one thread.
+//
+// The two polarisations of an antenna share the weights (one F-engine = the two pols of
+// one antenna) and, when their coarse delays are equal, the same column rotation (fe_fir.cuh explains
+// the rotation).  A thread then owns one complex FFT input point z[i] = g[2i] + i g[2i+1]
+// (PAPER.md:183), i.e. the two input columns 2i, 2i+1, for both pols, and the packed FP32 lanes hold
+// (pol 0, pol 1):
+//     acc[c][(r - j) mod T] (p0, p1) += s[r][c] (p0, p1) * w[c][j]          (w broadcast to both lanes)
+// which halves the weight registers of fe_fir.cuh (2*T instead of 4*T per 64 FMAs) and produces the
+// 16-byte unit {Re z p0, Re z p1, Im z p0, Im z p1} that the pol-packed FFT (fe_fft2.cuh) loads with
+// one 128-bit access.  Scratch row of (antenna, spectrum): n units = N*2 floats.
+//
+// Input staging is the ring of fe_fir.cuh with both pols' 80-byte row segments side by side in a
+// 160-byte slot.  A 5-byte group (4 samples) is shared by the two threads that own its two points.
+#pragma once
+#include "fe_common.cuh"
+#include "fe_fir.cuh"
+
+namespace fe {
+
+struct Fir2Params {
+    const uint8_t *in;        // [A][2][stream_bytes]
+    const float *weights;     // [N*T]
+    float *g;                 // scratch, row a*chunk_cap + (m - m_begin), n units of 16 bytes
+    const int32_t *coarse;    // [A*2][n_coarse]; the two pols of an antenna hold equal values
+    int64_t n_coarse;
+    int64_t stream_bytes;
+    int64_t rows_in;
+    int64_t m_begin, m_end;
+    int64_t chunk_cap;
+    int lgN;
+    int rows_per_tile;
+};
+
+constexpr int kFir2Threads = 128;
+constexpr int kFir2Warps = kFir2Threads / 32;
+constexpr int kFir2SegBytes = 80;                                   // per warp per row per pol: 16 groups x 5 bytes
+constexpr int kFir2SlotBytes = 2 * kFir2SegBytes;                   // both pols
+
+// Ring step q holds input row R0 + q of both pols, R0 = m0 - cq - 1; see fir_run in fe_fir.cuh for the
+// partial-sum bookkeeping, which is identical.
+template <int T, bool MIXED>
+__device__ __forceinline__ void fir2_run(const Fir2Params &prm, const uint8_t *wsrc, uint32_t ring_s, int64_t c,
+                                         int64_t m0, int n_out, int i_pt, float *grow0)
+{
+    constexpr int U = kFirUnroll;
+    static_assert(U % T == 0 && U % kFirDepth == 0, "unroll must cover whole tap and ring periods");
+    const int N = 1 << prm.lgN;
+    const int lane = threadIdx.x & 31;
+    const int cr = (int)(c & (int64_t)(N - 1));
+    const int64_t cq = (c - cr) >> prm.lgN;
+    const int v0 = 2 * i_pt;                                    // input columns v0 (Re z), v0 + 1 (Im z)
+
+    bool lagc[2];
+    float w0[T], w1[T];
+    {
+        int tc[2];
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const int t = v0 + i + cr;
+            lagc[i] = t >= N;
+            tc[i] = t & (N - 1);
+        }
+#pragma unroll
+        for (int j = 0; j < T; ++j) {
+            w0[j] = __ldg(prm.weights + tc[0] + (size_t)N * j);
+            w1[j] = __ldg(prm.weights + tc[1] + (size_t)N * j);
+        }
+    }
+    const int lag0 = lagc[0] ? 1 : 0;
+    const int64_t R0 = m0 - cq - 1;
+    const int row_bytes = N / 4 * 5;
+
+    // this thread's bytes in a slot: group gi = lane/2 of the warp's 16 groups, point e = lane&1 of the
+    // group: bytes [5 gi + e, 5 gi + e + 4) hold its two samples (bits 39..20 for e = 0, 19..0 for e = 1)
+    const int e = lane & 1;
+    const uint32_t boff = (uint32_t)(5 * (lane >> 1) + e);
+    const uint32_t sh = boff & 3;
+    const uint32_t sel = (sh + 3) | ((sh + 2) << 4) | ((sh + 1) << 8) | (sh << 12);
+    const uint32_t rd_addr = ring_s + (boff >> 2) * 4u;          // W0 of pol 0 in slot 0
+    const uint32_t sha = e ? 12u : 0u;                           // left shift that brings sample a to bits 31..22
+
+    // Batch copy: 4 rows x 2 pols x 5 chunks of 16 bytes = 40 chunks; lane l moves chunk l, lanes 0..7 also 32+l.
+    const int rowA = lane / 10, remA = lane - rowA * 10, polA = remA / 5, colA = remA - polA * 5;
+    const bool hasB = lane < 8;
+    const int rowB = 3, remB = hasB ? 2 + lane : 0, polB = remB / 5, colB = remB - polB * 5;
+    const uint32_t dstA = ring_s + (uint32_t)(rowA * kFir2SlotBytes + polA * kFir2SegBytes + colA * 16);
+    const uint32_t dstB = ring_s + (uint32_t)(rowB * kFir2SlotBytes + polB * kFir2SegBytes + colB * 16);
+    const uint8_t *srcA = wsrc + polA * prm.stream_bytes + (R0 + rowA) * (int64_t)row_bytes + colA * 16;
+    const uint8_t *srcB = wsrc + polB * prm.stream_bytes + (R0 + rowB) * (int64_t)row_bytes + colB * 16;
+    const int64_t batch_bytes = (int64_t)kFirBatch * row_bytes;
+    const int64_t lo64 = -R0, hi64 = prm.rows_in - R0;
+    const int q_lo = (int)max((int64_t)-0x3fffffff, min(lo64, (int64_t)0x3fffffff));
+    const int q_hi = (int)max((int64_t)-0x3fffffff, min(hi64, (int64_t)0x3fffffff));
+    const uint32_t span = (uint32_t)max(q_hi - q_lo, 0);
+    int tA = rowA - q_lo, tB = rowB - q_lo;
+
+    auto issue_batch = [&](int slot0) {
+        const uint32_t okA = (uint32_t)tA < span ? 1u : 0u;
+        const uint32_t okB = (uint32_t)tB < span ? 1u : 0u;
+        ring_fill(dstA + slot0 * kFir2SlotBytes, srcA, okA, okA ^ 1u);
+        ring_fill(dstB + slot0 * kFir2SlotBytes, srcB, hasB ? okB : 0u, hasB ? (okB ^ 1u) : 0u);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        srcA += batch_bytes;
+        srcB += batch_bytes;
+        tA += kFirBatch;
+        tB += kFirBatch;
+    };
+
+    __syncwarp();
+#pragma unroll
+    for (int b = 0; b < kFirRingBatches - 1; ++b) issue_batch(b * kFirBatch);
+
+    f2 acc0[T], acc1[T];                                        // columns v0, v0+1; lanes (pol 0, pol 1)
+#pragma unroll
+    for (int j = 0; j < T; ++j) acc0[j] = acc1[j] = f2(0.f, 0.f);
+    float4 prev = make_float4(0.f, 0.f, 0.f, 0.f);
+
+    const size_t g_stride = (size_t)N * 2;                      // next spectrum (floats): n units of 4 floats
+    float *gp = grow0 + 4 * i_pt + ((int64_t)(MIXED ? 0 : lag0) - T) * (int64_t)g_stride;
+    int sp = (MIXED ? 0 : lag0) - T;
+
+    const int n_steps = n_out + T;
+    for (int i0 = 0; i0 < n_steps; i0 += U) {
+#pragma unroll
+        for (int ii = 0; ii < U; ++ii) {
+            if (ii % kFirBatch == 0) {
+                cp_async_wait<kFirRingBatches - 2>();
+                __syncwarp();
+                issue_batch(((ii / kFirBatch + kFirRingBatches - 1) % kFirRingBatches) * kFirBatch);
+            }
+            const int slot = ii % kFirDepth;
+            uint32_t P0a, P0b, P1a, P1b;
+            const uint32_t ad = rd_addr + slot * kFir2SlotBytes;
+            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(P0a) : "r"(ad) : "memory");
+            asm volatile("ld.shared.u32 %0, [%1+4];" : "=r"(P0b) : "r"(ad) : "memory");
+            asm volatile("ld.shared.u32 %0, [%1+80];" : "=r"(P1a) : "r"(ad) : "memory");
+            asm volatile("ld.shared.u32 %0, [%1+84];" : "=r"(P1b) : "r"(ad) : "memory");
+            const uint32_t be0 = __byte_perm(P0a, P0b, sel) << sha;     // sample a in bits 31..22, b in 21..12
+            const uint32_t be1 = __byte_perm(P1a, P1b, sel) << sha;
+            const f2 s0((float)((int32_t)be0 >> 22), (float)((int32_t)be1 >> 22));                  // column v0, (p0, p1)
+            const f2 s1((float)((int32_t)(be0 << 10) >> 22), (float)((int32_t)(be1 << 10) >> 22));  // column v0 + 1
+            acc0[ii % T] = s0 * w0[0];
+            acc1[ii % T] = s1 * w1[0];
+#pragma unroll
+            for (int j = 1; j < T; ++j) {
+                acc0[(ii + T - j) % T] = fma_(s0, w0[j], acc0[(ii + T - j) % T]);
+                acc1[(ii + T - j) % T] = fma_(s1, w1[j], acc1[(ii + T - j) % T]);
+            }
+            const f2 d0 = acc0[(ii + 1) % T], d1 = acc1[(ii + 1) % T];
+            float4 cur = make_float4(d0.v.x, d0.v.y, d1.v.x, d1.v.y);       // {Re p0, Re p1, Im p0, Im p1}
+            if (MIXED) {
+                const float4 now = cur;
+                cur.x = lagc[0] ? prev.x : now.x;
+                cur.y = lagc[0] ? prev.y : now.y;
+                cur.z = lagc[1] ? prev.z : now.z;
+                cur.w = lagc[1] ? prev.w : now.w;
+                prev = now;
+            }
+            if ((unsigned)sp < (unsigned)n_out) *reinterpret_cast<float4 *>(gp) = cur;
+            gp += g_stride;
+            ++sp;
+        }
+    }
+    cp_async_wait<0>();
+}
+
+template <int T>
+__global__ void __launch_bounds__(kFir2Threads, 4) fir2_kernel(const Fir2Params prm)
+{
+    // +16: the second word of the last lane's pol-1 group may lie just past the last slot (never selected)
+    __shared__ __align__(16) unsigned char ring_all[kFir2Warps * kFirDepth * kFir2SlotBytes + 16];
+    const int N = 1 << prm.lgN;
+    const int a = blockIdx.z;
+    const int warp = threadIdx.x >> 5;
+    const int i_pt = blockIdx.x * kFir2Threads + threadIdx.x;   // complex point index 0..n-1
+    int64_t m = prm.m_begin + (int64_t)blockIdx.y * prm.rows_per_tile;
+    const int64_t m_stop = min(m + (int64_t)prm.rows_per_tile, prm.m_end);
+    const uint8_t *sbase = prm.in + (int64_t)a * 2 * prm.stream_bytes;
+    const uint8_t *wsrc = sbase + (int64_t)(blockIdx.x * kFir2Warps + warp) * kFir2SegBytes;
+    const int32_t *ctab = prm.coarse + (int64_t)a * 2 * prm.n_coarse;
+    const uint32_t ring_s = (uint32_t)__cvta_generic_to_shared(ring_all + warp * kFirDepth * kFir2SlotBytes);
+
+    while (m < m_stop) {
+        const int32_t c = ctab[prm.n_coarse == 1 ? 0 : m];
+        int64_t run_end = m_stop;
+        if (prm.n_coarse != 1) {
+            run_end = m + 1;
+            while (run_end < m_stop && ctab[run_end] == c) ++run_end;
+        }
+        float *grow0 = prm.g + ((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * (int64_t)N * 2;
+        const int cr = (int)((int64_t)c & (int64_t)(N - 1));
+        const bool mixed = (2 * i_pt + cr < N) && (2 * i_pt + 1 + cr >= N);
+        if (__any_sync(0xffffffffu, mixed))
+            fir2_run<T, true>(prm, wsrc, ring_s, (int64_t)c, m, (int)(run_end - m), i_pt, grow0);
+        else
+            fir2_run<T, false>(prm, wsrc, ring_s, (int64_t)c, m, (int)(run_end - m), i_pt, grow0);
+        m = run_end;
+    }
+}
+
+}  // namespace fe

@@ -18,7 +18,9 @@
 #include "../../include/fengine.h"
 #include "fe_common.cuh"
 #include "fe_fft.cuh"
+#include "fe_fft2.cuh"
 #include "fe_fir.cuh"
+#include "fe_fir2.cuh"
 #include "fe_generic.cuh"
 
 using namespace fe;
@@ -26,6 +28,9 @@ using namespace fe;
 struct fengine {
     int A = 0, n = 0, N = 0, lgN = 0, T = 0, P = 0;
     bool tiled = false;             // tiled kernels cover this (n, T)
+    bool packed_ok = false;         // pol-packed kernels (fe_fir2 / fe_fft2) cover this (n, T, P)
+    bool pols_equal = true;         // both pols of every antenna have equal coarse delays (needed by them)
+    bool allow_packed = true;       // option "pol_packed"
     int64_t n_coarse = 1, n_fine = 1;
     // device tables
     float *d_weights = nullptr;
@@ -33,6 +38,7 @@ struct fengine {
     float *d_fine_d = nullptr, *d_fine_phi = nullptr;
     float2 *d_gains = nullptr, *d_rg = nullptr;
     float4 *d_tw[3] = {nullptr, nullptr, nullptr};
+    float2 *d_tw1s = nullptr, *d_tw2s = nullptr;     // scalar twiddles of the pol-packed FFT
     float2 *d_tpost = nullptr;
     // scratch
     float *d_scratch = nullptr;
@@ -90,7 +96,13 @@ using Plan8192 = FftPlan<8192, 4, 8, 8, 8, 16, 256>;
 using Plan16384 = FftPlan<16384, 4, 16, 16, 8, 8, 512>;
 using Plan32768 = FftPlan<32768, 4, 32, 16, 8, 8, 512, 2>;     // two sweeps of 16384 points (fe_fft.cuh)
 
+using Plan2_1024 = Fft2Plan<1024, 8, 8, 64>;
+using Plan2_2048 = Fft2Plan<2048, 8, 16, 128>;
+using Plan2_4096 = Fft2Plan<4096, 16, 16, 256>;
+
 bool tiled_n(int n) { return n >= 1024 && n <= 32768; }
+bool packed_n(int n) { return n == 1024 || n == 2048 || n == 4096; }
+bool use_packed(const fengine *fe) { return fe->tiled && fe->packed_ok && fe->pols_equal && fe->allow_packed; }
 bool tiled_T(int T) { return T == 2 || T == 4 || T == 8 || T == 16; }
 
 template <class Plan>
@@ -104,6 +116,56 @@ int build_tables(fengine *fe)
     FE_CUDA(fe, cudaMalloc(&fe->d_tpost, sizeof(float2) * (size_t)Plan::n));
     build_post_twiddles<<<(Plan::n + 255) / 256, 256>>>(fe->d_tpost, Plan::n);
     FE_CUDA(fe, cudaGetLastError());
+    return FENGINE_OK;
+}
+
+template <class Plan>
+int build_tables2(fengine *fe)
+{
+    FE_CUDA(fe, cudaMalloc(&fe->d_tw1s, sizeof(float2) * (size_t)Plan::R1 * Plan::M1));
+    build_scalar_twiddles<<<(Plan::R1 * Plan::M1 + 255) / 256, 256>>>(fe->d_tw1s, Plan::R1, Plan::M1, Plan::n);
+    FE_CUDA(fe, cudaMalloc(&fe->d_tw2s, sizeof(float2) * (size_t)Plan::R2 * Plan::M2));
+    build_scalar_twiddles<<<(Plan::R2 * Plan::M2 + 255) / 256, 256>>>(fe->d_tw2s, Plan::R2, Plan::M2, Plan::M1);
+    FE_CUDA(fe, cudaGetLastError());
+    return FENGINE_OK;
+}
+
+template <class Plan, bool F32OUT>
+int launch_fft2(fengine *fe, const Fft2Params &prm, int64_t chunk_len, cudaStream_t stream)
+{
+    const size_t smem = fft2_smem_bytes<Plan>();
+    static bool attr_set = false;
+    if (!attr_set) {
+        FE_CUDA(fe, cudaFuncSetAttribute(fft2_kernel<Plan, F32OUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    dim3 grid((unsigned)chunk_len, (unsigned)fe->A);
+    fft2_kernel<Plan, F32OUT><<<grid, Plan::tpf, smem, stream>>>(prm);
+    return FENGINE_OK;
+}
+
+template <bool F32OUT>
+int launch_fft2_n(fengine *fe, const Fft2Params &prm, int64_t chunk_len, cudaStream_t stream)
+{
+    switch (fe->n) {
+    case 1024: return launch_fft2<Plan2_1024, F32OUT>(fe, prm, chunk_len, stream);
+    case 2048: return launch_fft2<Plan2_2048, F32OUT>(fe, prm, chunk_len, stream);
+    case 4096: return launch_fft2<Plan2_4096, F32OUT>(fe, prm, chunk_len, stream);
+    }
+    return fail(fe, FENGINE_ERR_INVALID_ARG, "no pol-packed FFT plan for n=%d", fe->n);
+}
+
+int launch_fir2(fengine *fe, const Fir2Params &prm, int64_t chunk_len, cudaStream_t stream)
+{
+    dim3 grid((unsigned)(fe->n / kFir2Threads), (unsigned)((chunk_len + prm.rows_per_tile - 1) / prm.rows_per_tile),
+              (unsigned)fe->A);
+    switch (fe->T) {
+    case 2: fir2_kernel<2><<<grid, kFir2Threads, 0, stream>>>(prm); break;
+    case 4: fir2_kernel<4><<<grid, kFir2Threads, 0, stream>>>(prm); break;
+    case 8: fir2_kernel<8><<<grid, kFir2Threads, 0, stream>>>(prm); break;
+    case 16: fir2_kernel<16><<<grid, kFir2Threads, 0, stream>>>(prm); break;
+    default: return fail(fe, FENGINE_ERR_INVALID_ARG, "no tiled FIR for T=%d", fe->T);
+    }
     return FENGINE_OK;
 }
 
@@ -277,10 +339,42 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
     xp.P = fe->P;
     xp.per_spectrum = per_spectrum ? 1 : 0;
 
+    const bool packed = use_packed(fe);
+    Fir2Params fp2{};
+    Fft2Params xp2{};
+    if (packed) {
+        fp2.in = fp.in;
+        fp2.weights = fp.weights;
+        fp2.g = fp.g;
+        fp2.coarse = fp.coarse;
+        fp2.n_coarse = fp.n_coarse;
+        fp2.stream_bytes = fp.stream_bytes;
+        fp2.rows_in = fp.rows_in;
+        fp2.chunk_cap = chunk;
+        fp2.lgN = fe->lgN;
+        fp2.rows_per_tile = fe->fir_rows;
+        xp2.g = fe->d_scratch;
+        xp2.out = out;
+        xp2.out_f32 = out_f32;
+        xp2.tw1 = fe->d_tw1s;
+        xp2.tw2 = fe->d_tw2s;
+        xp2.tpost = fe->d_tpost;
+        xp2.rg = fe->d_rg;
+        xp2.gains = fe->d_gains;
+        xp2.coarse = fe->d_coarse;
+        xp2.fine_d = fe->d_fine_d;
+        xp2.fine_phi = fe->d_fine_phi;
+        xp2.n_coarse = fe->n_coarse;
+        xp2.n_fine = fe->n_fine;
+        xp2.chunk_cap = chunk;
+        xp2.n_spectra = S;
+        xp2.per_spectrum = per_spectrum ? 1 : 0;
+    }
+
     for (int64_t m0 = 0; m0 < S; m0 += chunk) {
         const int64_t m1 = std::min(S, m0 + chunk);
-        fp.m_begin = xp.m_begin = m0;
-        fp.m_end = xp.m_end = m1;
+        fp.m_begin = xp.m_begin = fp2.m_begin = xp2.m_begin = m0;
+        fp.m_end = xp.m_end = fp2.m_end = xp2.m_end = m1;
         cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
         if (fe->profile) {
             for (auto &e : ev) {
@@ -294,10 +388,13 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
             }
             FE_CUDA(fe, cudaEventRecord(ev[0], stream));
         }
-        rc = launch_fir(fe, fp, m1 - m0, stream);
+        rc = packed ? launch_fir2(fe, fp2, m1 - m0, stream) : launch_fir(fe, fp, m1 - m0, stream);
         if (rc) return rc;
         if (fe->profile) FE_CUDA(fe, cudaEventRecord(ev[1], stream));
-        rc = out_f32 ? launch_fft_n<true>(fe, xp, m1 - m0, stream) : launch_fft_n<false>(fe, xp, m1 - m0, stream);
+        if (packed)
+            rc = out_f32 ? launch_fft2_n<true>(fe, xp2, m1 - m0, stream) : launch_fft2_n<false>(fe, xp2, m1 - m0, stream);
+        else
+            rc = out_f32 ? launch_fft_n<true>(fe, xp, m1 - m0, stream) : launch_fft_n<false>(fe, xp, m1 - m0, stream);
         if (rc) return rc;
         if (fe->profile) FE_CUDA(fe, cudaEventRecord(ev[2], stream));
         fe->last_launches += 2;
@@ -357,6 +454,14 @@ fengine_t *fengine_create_batched(int n_antennas, int n_channels, int taps, int 
         case 16384: rc = build_tables<Plan16384>(fe); break;
         case 32768: rc = build_tables<Plan32768>(fe); break;
         }
+        fe->packed_ok = rc == FENGINE_OK && fe->P == 2 && packed_n(fe->n);
+        if (fe->packed_ok) {
+            switch (fe->n) {
+            case 1024: rc = build_tables2<Plan2_1024>(fe); break;
+            case 2048: rc = build_tables2<Plan2_2048>(fe); break;
+            case 4096: rc = build_tables2<Plan2_4096>(fe); break;
+            }
+        }
         ok = rc == FENGINE_OK;
     }
     if (ok) ok = cudaDeviceSynchronize() == cudaSuccess;
@@ -385,6 +490,8 @@ void fengine_destroy(fengine_t *fe)
     cudaFree(fe->d_rg);
     for (auto &t : fe->d_tw) cudaFree(t);
     cudaFree(fe->d_tpost);
+    cudaFree(fe->d_tw1s);
+    cudaFree(fe->d_tw2s);
     cudaFree(fe->d_scratch);
     cudaFree(fe->d_stage_in);
     cudaFree(fe->d_stage_out);
@@ -413,6 +520,11 @@ int fengine_set_coarse_delays(fengine_t *fe, const int32_t *c, int64_t n_per_str
         fe->n_coarse = n_per_stream;
     }
     FE_CUDA(fe, cudaMemcpy(fe->d_coarse, c, sizeof(int32_t) * count, cudaMemcpyHostToDevice));
+    fe->pols_equal = true;                                  // the pol-packed kernels share one delay per antenna
+    if (fe->P == 2)
+        for (int a = 0; a < fe->A && fe->pols_equal; ++a)
+            fe->pols_equal = memcmp(c + (size_t)(2 * a) * n_per_stream, c + (size_t)(2 * a + 1) * n_per_stream,
+                                    sizeof(int32_t) * (size_t)n_per_stream) == 0;
     fe->rg_dirty = true;
     return FENGINE_OK;
 }
@@ -531,6 +643,26 @@ int fengine_debug_fir(fengine_t *fe, const void *in, float *g_out, int64_t n_spe
     const int64_t total = (int64_t)fe->A * fe->P * n_spectra * fe->N;
     if (!fe->tiled) {
         gen_fir_kernel<<<gen_grid(total), 256, 0, s>>>(gen_params(fe, in, n_spectra), g_out);
+    } else if (use_packed(fe)) {
+        rc = ensure_scratch(fe, (size_t)total);
+        if (rc) return rc;
+        Fir2Params fp{};
+        fp.in = static_cast<const uint8_t *>(in);
+        fp.weights = fe->d_weights;
+        fp.g = fe->d_scratch;
+        fp.coarse = fe->d_coarse;
+        fp.n_coarse = fe->n_coarse;
+        fp.rows_in = n_spectra + fe->T - 1;
+        fp.stream_bytes = (int64_t)fe->N * fp.rows_in / 4 * 5;
+        fp.m_begin = 0;
+        fp.m_end = n_spectra;
+        fp.chunk_cap = n_spectra;
+        fp.lgN = fe->lgN;
+        fp.rows_per_tile = fe->fir_rows;
+        rc = launch_fir2(fe, fp, n_spectra, s);
+        if (rc) return rc;
+        unrotate2_kernel<<<gen_grid(total), 256, 0, s>>>(fe->d_scratch, g_out, fe->d_coarse, fe->n_coarse, n_spectra,
+                                                         n_spectra, fe->N, fe->A);
     } else {
         rc = ensure_scratch(fe, (size_t)total);
         if (rc) return rc;
@@ -575,6 +707,10 @@ int fengine_set_option(fengine_t *fe, const char *key, int64_t value)
     }
     if (!strcmp(key, "profile")) {
         fe->profile = value != 0;
+        return FENGINE_OK;
+    }
+    if (!strcmp(key, "pol_packed")) {
+        fe->allow_packed = value != 0;
         return FENGINE_OK;
     }
     if (!strcmp(key, "force_generic")) {
