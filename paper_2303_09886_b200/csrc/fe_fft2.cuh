@@ -6,15 +6,13 @@
 // n = R1*R2*R3 with R1 = 16, decimation in frequency, natural-order input:
 //   pass 1, 2   packed FP32 lanes = (pol 0, pol 1): one butterfly serves both pols and every twiddle is a
 //               scalar broadcast to both lanes, so the twiddle tables are read once per spectrum, not per pol;
-//   pass 3      scalar, thread = (residue pair K / Q-K, pol): it owns Z[k] and Z[n-k] of its pol and does the
-//               real-FFT post-twiddle (the paper's kernel also ran "two such FFTs ... by the
-//               same thread"), the rotation, the gain and the quantisation in registers; the two
-//               pols of a channel sit in neighbouring lanes and are joined by one shuffle into the 4-byte
-//               output word {re0, im0, re1, im1}.
+//   pass 3      thread K transforms residue K (Z[K + Q kq]), swaps the upper half of its outputs with the thread of
+//               the mirror residue Q - K through the exchange buffer, and then owns Z[k] and Z[n-k] for half of
+//               its channels: real-FFT post-twiddle, rotation, gain, quantisation and the 4-byte
+//               output word {re0, im0, re1, im1} of a channel all happen in registers, packed over the pols.
 // Exchange buffer (in place, one __syncthreads per pass): unit (k1, rest) lives at k1*(n/16 + 1) + rest.
-// The one-unit skew per k1 block makes the scalar 64-bit reads of pass 3 (16 lanes = 16 consecutive k1)
-// bank-conflict free; pass 2 writes each unit as {re0, im0, re1, im1} so that pass 3 reads (re, im) of its
-// pol with one 64-bit load.
+// The one-unit skew per k1 block makes the 128-bit accesses of pass 3 (consecutive lanes = consecutive k1)
+// bank-conflict free.
 #pragma once
 #include "fe_common.cuh"
 #include "fe_fft.cuh"
@@ -34,7 +32,7 @@ struct Fft2Plan {
     static_assert(R1 * R2_ * R3_ == N_CH, "radices must multiply to n");
     static_assert(M2 == R3_, "three passes");
     static_assert(R3_ == 8 || R3_ == 16, "last radix 8 or 16");
-    static_assert(Q % 32 == 0 && TPF % 32 == 0 && TPF >= 64, "whole warps in the last pass");
+    static_assert(TPF == Q && TPF % 32 == 0 && TPF >= 64, "one residue per thread in the last pass");
 };
 
 struct Fft2Params {
@@ -44,8 +42,7 @@ struct Fft2Params {
     const float2 *tw1;        // [16][M1]  W_n^{k col}   (cos, -sin)
     const float2 *tw2;        // [R2][M2]  W_M1^{k lo}
     const float2 *tpost;      // [n] (sin, cos)(2 pi k / N)  =  i * exp(-2 pi i k / N)
-    const float2 *rg;         // const mode: [A][2][n]  0.5 * G * exp(i(-2 pi (d + cr) k/N + phi))
-    const float2 *gains;      // per-spectrum mode: [A][2][n]
+    const float4 *rg2;        // [A][n] {re p0, re p1, im p0, im p1}: const mode 0.5 * G * rotation; per-spectrum mode G
     const int32_t *coarse;    // [A*2][n_coarse]
     const float *fine_d;      // [A*2][n_fine]
     const float *fine_phi;    // [A*2][n_fine]
@@ -101,139 +98,151 @@ __device__ __forceinline__ void fft2_pass2(float4 *sm, const float2 *__restrict_
                 const float2 w = __ldg(tw + k * M2 + lo);
                 y = cmul(x[k], w.x, w.y);
             }
-            col[k * M2] = make_float4(y.re.v.x, y.im.v.x, y.re.v.y, y.im.v.y);     // {re0, im0, re1, im1}
+            col[k * M2] = make_float4(y.re.v.x, y.re.v.y, y.im.v.x, y.im.v.y);
         }
     }
 }
 
-// residue K of pol p -> Z[K + Q kq], kq = 0..R3-1 (scalar butterfly)
-template <class Plan>
-__device__ __forceinline__ void fft2_load_residue(const float4 *sm, int K, int p, cx<float> (&z)[Plan::R3])
+struct SpectrumPhase2 {      // shared, filled once per spectrum in per-spectrum mode; packed {re p0, re p1, im p0, im p1}
+    float4 step[16];         // exp(-2 pi i d_eff Q kq / N)
+    float4 c3;               // exp(2 i phi) exp(-i pi d_eff): E[n-k] = c3 * conj(E[k]) with E incl. exp(i phi)
+    float4 ephi;             // exp(i phi)
+};
+
+__device__ __forceinline__ cx<f2> unpack_unit(float4 v) { return {f2(v.x, v.y), f2(v.z, v.w)}; }
+__device__ __forceinline__ float4 pack_unit(cx<f2> z) { return make_float4(z.re.v.x, z.re.v.y, z.im.v.x, z.im.v.y); }
+// packed complex product (both lanes independent)
+__device__ __forceinline__ cx<f2> cmul2(cx<f2> a, cx<f2> b)
 {
-    const int k1 = K & (Plan::R1 - 1), k2 = K / Plan::R1;
-    const float2 *src = reinterpret_cast<const float2 *>(sm + k1 * Plan::blk + k2 * Plan::M2) + p;
-#pragma unroll
-    for (int t = 0; t < Plan::R3; ++t) {
-        const float2 v = src[2 * t];
-        z[t] = {v.x, v.y};
-    }
-    Dif<Plan::R3, float>::run(z);
+    return {fnma_(a.im, b.im, a.re * b.re), fma_(a.im, b.re, a.re * b.im)};
 }
 
+// {re p0, im p0, re p1, im p1} int8 word: round-half-even + clamp to [-127, 127]
+__device__ __forceinline__ uint32_t quantize_unit(cx<f2> y)
+{
+    const float magic = 12582912.0f;                      // 1.5 * 2^23: the FP32 add rounds to nearest-even
+    const f2 r = f2(fminf(fmaxf(y.re.v.x, -127.0f), 127.0f), fminf(fmaxf(y.re.v.y, -127.0f), 127.0f)) + f2(magic);
+    const f2 i = f2(fminf(fmaxf(y.im.v.x, -127.0f), 127.0f), fminf(fmaxf(y.im.v.y, -127.0f), 127.0f)) + f2(magic);
+    const uint32_t lo = __byte_perm(__float_as_uint(r.v.x), __float_as_uint(i.v.x), 0x0040);
+    const uint32_t hi = __byte_perm(__float_as_uint(r.v.y), __float_as_uint(i.v.y), 0x0040);
+    return __byte_perm(lo, hi, 0x5410);
+}
+
+// Post-twiddle, rotation, gain and store of channel kA = K + Q kq and of its mirror n - kA,
+// both pols in the packed lanes.  zk = Z[kA], zm = Z[n - kA]; tp = i w^kA; rgA / rgB = 0.5 * gain * rotation.
+template <bool F32OUT>
+__device__ __forceinline__ void fft2_epilogue(cx<f2> zk, cx<f2> zm, float2 tp, cx<f2> rgA, cx<f2> rgB, int kA, int kB,
+                                              int n, uint32_t *rec, float4 *yout)
+{
+    const f2 sr = zk.re + zm.re, si = zk.im - zm.im;      // S = Z[k] + conj Z[n-k]
+    const f2 dr = zk.re - zm.re, di = zk.im + zm.im;      // D = Z[k] - conj Z[n-k]
+    const f2 fr = fnma_(di, tp.y, dr * tp.x);             // F = D * (i w^k)
+    const f2 fi = fma_(di, tp.x, dr * tp.y);
+    const cx<f2> xk = {sr - fr, si - fi};                 // 2 X[k]
+    const cx<f2> xm = {sr + fr, -(si + fi)};              // 2 X[n-k] = conj(S + F)
+    const cx<f2> yA = cmul2(xk, rgA), yB = cmul2(xm, rgB);
+    if (F32OUT) {
+        yout[kA] = make_float4(yA.re.v.x, yA.im.v.x, yA.re.v.y, yA.im.v.y);
+        if (kB < n) yout[kB] = make_float4(yB.re.v.x, yB.im.v.x, yB.re.v.y, yB.im.v.y);
+    } else {
+        rec[kA] = quantize_unit(yA);
+        if (kB < n) rec[kB] = quantize_unit(yB);
+    }
+}
+
+// Pass 3: thread K transforms residue K (packed radix-R3 butterfly, Z[K + Q kq]), hands the upper half of its
+// outputs to the thread of the mirror residue Q - K through the exchange buffer (in place, its own slots), and
+// finishes the channels K + Q kq, kq < R3/2, together with their mirrors n - k, whose Z values are exactly the
+// upper half of residue Q - K.  Residue 0 mirrors onto itself with the index shifted by one (n - Q kq = Q (R3 - kq))
+// and also owns the self-mirrored channel n/2.
 template <class Plan, bool F32OUT>
-__device__ __forceinline__ void fft2_pass3(const float4 *sm, const Fft2Params &prm, int a, int64_t m, int tid,
-                                           const SpectrumPhase *sph_all, const double (&dts_p)[2], const int (&cr_p)[2])
+__device__ __forceinline__ void fft2_pass3(float4 *sm, const Fft2Params &prm, int a, int64_t m, int tid,
+                                           const SpectrumPhase2 *sph)
 {
-    constexpr int Rq = Plan::R3, Q = Plan::Q, n = Plan::n, N = 2 * n;
+    constexpr int R = Plan::R3, H = R / 2, Q = Plan::Q, n = Plan::n, N = 2 * n;
+    static_assert(Plan::tpf == Q, "one residue per thread");
+    const int K = tid;
+    float4 *mine = sm + (K & (Plan::R1 - 1)) * Plan::blk + (K / Plan::R1) * Plan::M2;
+    const int Kp = (Q - K) & (Q - 1);
+    const float4 *theirs = sm + (Kp & (Plan::R1 - 1)) * Plan::blk + (Kp / Plan::R1) * Plan::M2;
+
+    cx<f2> z[R];
+#pragma unroll
+    for (int t = 0; t < R; ++t) z[t] = unpack_unit(mine[t]);
+    Dif<R, f2>::run(z);
+    if (K == 0) {
+#pragma unroll
+        for (int j = 0; j < H; ++j) mine[j] = pack_unit(z[(R - j) % R]);
+        mine[H] = pack_unit(z[H]);
+    } else {
+#pragma unroll
+        for (int j = 0; j < H; ++j) mine[j] = pack_unit(z[R - 1 - j]);
+    }
+
+    // per-thread rotation base of the per-spectrum mode: E_p(K) = exp(i phi_p) exp(-2 pi i (d_p + cr) K / N)
+    cx<f2> base = {f2(1.f, 1.f), f2(0.f, 0.f)};
+    const float4 *__restrict__ gtab = reinterpret_cast<const float4 *>(prm.rg2) + (int64_t)a * n;
+    if (prm.per_spectrum) {
+        float2 e[2];
+#pragma unroll
+        for (int p = 0; p < 2; ++p) {
+            const int64_t st = (int64_t)a * 2 + p;
+            const int32_t c = prm.coarse[st * prm.n_coarse + (prm.n_coarse == 1 ? 0 : m)];
+            const int cr = (int)(c & (N - 1));
+            const double d = (double)prm.fine_d[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
+            const double phi = (double)prm.fine_phi[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
+            const double t = -(d / (double)N) * (double)K - (double)((cr * K) & (N - 1)) / (double)N;
+            double sp_, cp_;
+            sincos(phi, &sp_, &cp_);
+            e[p] = cmulf(phasor_turns(t), make_float2((float)cp_, (float)sp_));
+        }
+        base = {f2(e[0].x, e[1].x), f2(e[0].y, e[1].y)};
+    }
     const float2 *__restrict__ tpost = prm.tpost;
-    for (int it = tid; it < Q; it += Plan::tpf) {
-        const int p = it & 1, pidx = it >> 1;
-        const int64_t st = (int64_t)a * 2 + p;
-        const float2 *__restrict__ gtab = (prm.per_spectrum ? prm.gains : prm.rg) + st * n;
-        const SpectrumPhase *sph = sph_all + p;
-        const double d_eff_turn_scale = dts_p[p];
-        const int cr = cr_p[p];
-        cx<float> zA[Rq], zB[Rq];
-        const bool special = pidx == 0;
-        fft2_load_residue<Plan>(sm, pidx, p, zA);
-        fft2_load_residue<Plan>(sm, special ? Q / 2 : Q - pidx, p, zB);
+    uint32_t *rec = F32OUT ? nullptr : reinterpret_cast<uint32_t *>(prm.out + (((int64_t)a * prm.n_spectra + m) * n) * 4);
+    float4 *yout = F32OUT ? reinterpret_cast<float4 *>(prm.out_f32 + (((int64_t)a * prm.n_spectra + m) * n) * 4) : nullptr;
 
-        cx<float> zhalf = zA[Rq / 2];                     // only meaningful for the special thread
-        if (special) {                                    // residues 0 and Q/2 mirror onto themselves: re-pair
-            cx<float> a_[Rq], b_[Rq];
-#pragma unroll
-            for (int i = 0; i < Rq; ++i) { a_[i] = zA[i]; b_[i] = zB[i]; }
-#pragma unroll
-            for (int i = 0; i < Rq / 2; ++i) {
-                zA[i] = a_[i];
-                zA[Rq / 2 + i] = b_[i];
-                zB[i] = b_[Rq / 2 + i];
-            }
-#pragma unroll
-            for (int j = Rq / 2; j < Rq - 1; ++j) zB[j] = a_[j + 1];
-            zB[Rq - 1] = a_[0];
-        }
-
-        float2 base = make_float2(1.f, 0.f), base2 = make_float2(1.f, 0.f);
+    auto rot_gain = [&](int kq, int kA, int kB, cx<f2> &rgA, cx<f2> &rgB) {
+        const cx<f2> gA = unpack_unit(__ldg(gtab + kA));
+        const cx<f2> gB = unpack_unit(__ldg(gtab + (kB & (n - 1))));
         if (prm.per_spectrum) {
-            auto E_of = [&](int k) {                      // exp(i phi) exp(-2 pi i d_eff k / N), d_eff = d + cr
-                const double t = -d_eff_turn_scale * (double)k - (double)((cr * k) & (N - 1)) / (double)N;
-                return cmulf(phasor_turns(t), sph->ephi);
-            };
-            base = E_of(pidx);
-            if (special) base2 = E_of(Q / 2);
+            const cx<f2> E = cmul2(base, unpack_unit(sph->step[kq]));
+            const cx<f2> Ec = {E.re, -E.im};
+            const cx<f2> eA = {E.re * 0.5f, E.im * 0.5f};
+            const cx<f2> c3 = unpack_unit(sph->c3);
+            const cx<f2> eB0 = cmul2(c3, Ec);
+            const cx<f2> eB = {eB0.re * 0.5f, eB0.im * 0.5f};
+            rgA = cmul2(eA, gA);
+            rgB = cmul2(eB, gB);
+        } else {
+            rgA = gA;
+            rgB = gB;
         }
+    };
 
-        float *yout = nullptr;
-        uint32_t *rec = nullptr;
-        if (F32OUT) yout = prm.out_f32 + (((int64_t)a * prm.n_spectra + m) * n) * 4 + p * 2;
-        else rec = reinterpret_cast<uint32_t *>(prm.out + (((int64_t)a * prm.n_spectra + m) * n) * 4);
-
+    __syncthreads();                                      // upper halves are in the exchange buffer
+    cx<f2> zm[H];
 #pragma unroll
-        for (int kq = 0; kq < Rq; ++kq) {
-            const int kA = special ? (kq < Rq / 2 ? Q * kq : Q / 2 + Q * (kq - Rq / 2)) : pidx + Q * kq;
-            const int kB = n - kA;                        // == n for the DC pair (dropped Nyquist)
-            const cx<float> zk = zA[kq], zm = zB[Rq - 1 - kq];
-            const float2 tp = __ldg(tpost + kA);          // i w^k = (sin, cos)(2 pi k / N)
-            const float sr = zk.re + zm.re, si = zk.im - zm.im;     // S = Z[k] + conj Z[n-k]
-            const float dr = zk.re - zm.re, di = zk.im + zm.im;     // D = Z[k] - conj Z[n-k]
-            const float fr = fmaf(-di, tp.y, dr * tp.x);            // F = D * (i w^k)
-            const float fi = fmaf(di, tp.x, dr * tp.y);
-            const float xkr = sr - fr, xki = si - fi;               // 2 X[k]
-            const float xmr = sr + fr, xmi = -(si + fi);            // 2 X[n-k] = conj(S + F)
-            float2 rgA, rgB;
-            if (prm.per_spectrum) {
-                const bool hi = special && kq >= Rq / 2;
-                const float2 stp = sph->step[hi ? kq - Rq / 2 : kq];
-                const float2 E = cmulf(hi ? base2 : base, stp);
-                const float2 gA = __ldg(gtab + kA);
-                const float2 gB = __ldg(gtab + (kB & (n - 1)));
-                rgA = cmulf(E, gA);
-                rgB = cmulf(cmulf(sph->c3, make_float2(E.x, -E.y)), gB);
-                rgA.x *= 0.5f; rgA.y *= 0.5f; rgB.x *= 0.5f; rgB.y *= 0.5f;
-            } else {
-                rgA = __ldg(gtab + kA);
-                rgB = __ldg(gtab + (kB & (n - 1)));
-            }
-            const float yAr = fmaf(-xki, rgA.y, xkr * rgA.x), yAi = fmaf(xki, rgA.x, xkr * rgA.y);
-            const float yBr = fmaf(-xmi, rgB.y, xmr * rgB.x), yBi = fmaf(xmi, rgB.x, xmr * rgB.y);
-            if (F32OUT) {
-                *reinterpret_cast<float2 *>(yout + (int64_t)kA * 4) = make_float2(yAr, yAi);
-                if (kB < n) *reinterpret_cast<float2 *>(yout + (int64_t)kB * 4) = make_float2(yBr, yBi);
-            } else {
-                // lane p = 0 stores channel kA, lane p = 1 channel kB; each fetches the other pol from its neighbour
-                const uint32_t qA = quantize_pair(yAr, yAi), qB = quantize_pair(yBr, yBi);
-                const uint32_t other = __shfl_xor_sync(0xffffffffu, p ? qA : qB, 1);
-                if (p == 0) rec[kA] = __byte_perm(qA, other, 0x5410);            // {re0, im0, re1, im1}
-                else if (kB < n) rec[kB] = __byte_perm(other, qB, 0x5410);
-            }
-        }
-        if ((it & ~31) == 0) {                            // channel n/2: X = conj Z[n/2] (special lanes; warp-uniform branch)
-            float2 rg;
-            if (prm.per_spectrum) {
-                const float2 E = cmulf(sph->ephi, sph->step[Rq / 2]);   // k = Q * Rq/2 = n/2
-                rg = cmulf(E, __ldg(gtab + n / 2));
-            } else {
-                const float2 t = __ldg(gtab + n / 2);
-                rg = make_float2(2.f * t.x, 2.f * t.y);                // table holds 0.5 * ...
-            }
-            const float xr = zhalf.re, xi = -zhalf.im;
-            const float yr = fmaf(-xi, rg.y, xr * rg.x), yi = fmaf(xi, rg.x, xr * rg.y);
-            if (F32OUT) {
-                if (special) *reinterpret_cast<float2 *>(yout + (int64_t)(n / 2) * 4) = make_float2(yr, yi);
-            } else {
-                const uint32_t qh = quantize_pair(yr, yi);
-                const uint32_t other = __shfl_xor_sync(0xffffffffu, qh, 1);
-                if (special && p == 0) rec[n / 2] = __byte_perm(qh, other, 0x5410);
-            }
-        }
+    for (int j = 0; j < H; ++j) zm[j] = unpack_unit(theirs[j]);
+#pragma unroll
+    for (int kq = 0; kq < H; ++kq) {
+        const int kA = K + Q * kq, kB = n - kA;            // kB == n for the DC channel (dropped Nyquist)
+        cx<f2> rgA, rgB;
+        rot_gain(kq, kA, kB, rgA, rgB);
+        fft2_epilogue<F32OUT>(z[kq], zm[kq], __ldg(tpost + kA), rgA, rgB, kA, kB, n, rec, yout);
+    }
+    if (K == 0) {                                         // channel n/2 = Q * H mirrors onto itself
+        const cx<f2> zh = unpack_unit(mine[H]);
+        cx<f2> rgA, rgB;
+        rot_gain(H, n / 2, n / 2, rgA, rgB);
+        fft2_epilogue<F32OUT>(zh, zh, __ldg(tpost + n / 2), rgA, rgB, n / 2, n, n, rec, yout);
     }
 }
 
 template <class Plan>
 constexpr size_t fft2_smem_bytes()
 {
-    return (size_t)Plan::units * 16 + 2 * sizeof(SpectrumPhase);
+    return (size_t)Plan::units * 16 + sizeof(SpectrumPhase2);
 }
 
 // One CTA per (antenna, spectrum), both pols.
@@ -243,7 +252,7 @@ __global__ void __launch_bounds__(Plan::tpf, (512 / Plan::tpf) > 0 ? (512 / Plan
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int n = Plan::n, N = 2 * n;
     float4 *sm = reinterpret_cast<float4 *>(smem_raw);
-    SpectrumPhase *sph = reinterpret_cast<SpectrumPhase *>(smem_raw + (size_t)Plan::units * 16);
+    SpectrumPhase2 *sph = reinterpret_cast<SpectrumPhase2 *>(smem_raw + (size_t)Plan::units * 16);
 
     const int tid = threadIdx.x;
     const int a = blockIdx.y;
@@ -252,31 +261,35 @@ __global__ void __launch_bounds__(Plan::tpf, (512 / Plan::tpf) > 0 ? (512 / Plan
 
     const float4 *grow = reinterpret_cast<const float4 *>(prm.g + ((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * (int64_t)N * 2);
 
-    double dts[2] = {0.0, 0.0};
-    int cr[2] = {0, 0};
-    if (prm.per_spectrum) {
-#pragma unroll
-        for (int p = 0; p < 2; ++p) {
+    if (prm.per_spectrum) {                               // warp p sets up pol p's phasors
+        const int p = tid >> 5, t = tid & 31;
+        if (p < 2 && t <= 16) {
             const int64_t st = (int64_t)a * 2 + p;
             const int32_t c = prm.coarse[st * prm.n_coarse + (prm.n_coarse == 1 ? 0 : m)];
-            cr[p] = (int)(c & (N - 1));
+            const int cr = (int)(c & (N - 1));
             const double d = (double)prm.fine_d[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
             const double phi = (double)prm.fine_phi[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
-            dts[p] = d / (double)N;
-            const int t = tid - 32 * p;                   // warp p sets up pol p
-            if (t >= 0 && t < 16) {
+            if (t < 16) {
                 const int k = Plan::Q * t;
-                const double tt = -dts[p] * (double)k - (double)((cr[p] * k) & (N - 1)) / (double)N;
-                sph[p].step[t] = phasor_turns(tt);
-            } else if (t == 16) {
+                const double tt = -(d / (double)N) * (double)k - (double)((cr * k) & (N - 1)) / (double)N;
+                const float2 v = phasor_turns(tt);
+                float *dst = reinterpret_cast<float *>(&sph->step[t]);
+                dst[p] = v.x;
+                dst[2 + p] = v.y;
+            } else {
                 double s, c_;
                 sincos(phi, &s, &c_);
-                sph[p].ephi = make_float2((float)c_, (float)s);
+                float *de = reinterpret_cast<float *>(&sph->ephi);
+                de[p] = (float)c_;
+                de[2 + p] = (float)s;
                 sincos(2.0 * phi, &s, &c_);
                 const float2 e2 = make_float2((float)c_, (float)s);
                 float2 h = phasor_turns(-0.5 * d);        // exp(-i pi d_eff) = exp(-i pi d) * (-1)^cr
-                if (cr[p] & 1) { h.x = -h.x; h.y = -h.y; }
-                sph[p].c3 = cmulf(e2, h);
+                if (cr & 1) { h.x = -h.x; h.y = -h.y; }
+                const float2 c3 = cmulf(e2, h);
+                float *dc = reinterpret_cast<float *>(&sph->c3);
+                dc[p] = c3.x;
+                dc[2 + p] = c3.y;
             }
         }
     }
@@ -285,7 +298,39 @@ __global__ void __launch_bounds__(Plan::tpf, (512 / Plan::tpf) > 0 ? (512 / Plan
     __syncthreads();
     fft2_pass2<Plan>(sm, prm.tw2, tid);
     __syncthreads();
-    fft2_pass3<Plan, F32OUT>(sm, prm, a, m, tid, sph, dts, cr);
+    fft2_pass3<Plan, F32OUT>(sm, prm, a, m, tid, sph);
+}
+
+// Pol-interleaved table of the pol-packed epilogue, [A][n] units {re p0, re p1, im p0, im p1}:
+//   const mode          0.5 * G * exp(i(-2 pi (d + cr) k / N + phi))   (rotation folded in)
+//   per-spectrum mode   G                                              (rotation computed per spectrum in the kernel)
+__global__ void build_rg2_table(float4 *rg2, const float2 *gains, const int32_t *coarse, const float *fine_d,
+                                const float *fine_phi, int n, int A, int per_spectrum)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int a = blockIdx.y;
+    if (k >= n || a >= A) return;
+    const int N = 2 * n;
+    float re[2], im[2];
+    for (int p = 0; p < 2; ++p) {
+        const int st = a * 2 + p;
+        const float2 g = gains[(int64_t)st * n + k];
+        if (per_spectrum) {
+            re[p] = g.x;
+            im[p] = g.y;
+        } else {
+            const int cr = (int)(coarse[st] & (N - 1));
+            const double d = (double)fine_d[st], phi = (double)fine_phi[st];
+            const double turns = -d * (double)k / (double)N - (double)(((int64_t)cr * k) & (N - 1)) / (double)N;
+            double s, c, sp, cp;
+            sincospi(2.0 * turns, &s, &c);
+            sincos(phi, &sp, &cp);
+            const double rr = c * cp - s * sp, ri = c * sp + s * cp;
+            re[p] = (float)(0.5 * ((double)g.x * rr - (double)g.y * ri));
+            im[p] = (float)(0.5 * ((double)g.x * ri + (double)g.y * rr));
+        }
+    }
+    rg2[(int64_t)a * n + k] = make_float4(re[0], re[1], im[0], im[1]);
 }
 
 // scalar twiddle table of one pass: tw[k][x] = W_M^{k x} = (cos, -sin)(2 pi k x / M)

@@ -39,6 +39,8 @@ struct fengine {
     float2 *d_gains = nullptr, *d_rg = nullptr;
     float4 *d_tw[3] = {nullptr, nullptr, nullptr};
     float2 *d_tw1s = nullptr, *d_tw2s = nullptr;     // scalar twiddles of the pol-packed FFT
+    float4 *d_rg2 = nullptr;                         // pol-interleaved gain (x rotation) table of the pol-packed FFT
+    int rg2_mode = -1;                               // -1 stale, 0 const mode, 1 per-spectrum mode
     float2 *d_tpost = nullptr;
     // scratch
     float *d_scratch = nullptr;
@@ -96,7 +98,7 @@ using Plan8192 = FftPlan<8192, 4, 8, 8, 8, 16, 256>;
 using Plan16384 = FftPlan<16384, 4, 16, 16, 8, 8, 512>;
 using Plan32768 = FftPlan<32768, 4, 32, 16, 8, 8, 512, 2>;     // two sweeps of 16384 points (fe_fft.cuh)
 
-using Plan2_1024 = Fft2Plan<1024, 8, 8, 64>;
+using Plan2_1024 = Fft2Plan<1024, 8, 8, 128>;
 using Plan2_2048 = Fft2Plan<2048, 8, 16, 128>;
 using Plan2_4096 = Fft2Plan<4096, 16, 16, 256>;
 
@@ -124,6 +126,7 @@ int build_tables2(fengine *fe)
 {
     FE_CUDA(fe, cudaMalloc(&fe->d_tw1s, sizeof(float2) * (size_t)Plan::R1 * Plan::M1));
     build_scalar_twiddles<<<(Plan::R1 * Plan::M1 + 255) / 256, 256>>>(fe->d_tw1s, Plan::R1, Plan::M1, Plan::n);
+    FE_CUDA(fe, cudaMalloc(&fe->d_rg2, sizeof(float4) * (size_t)fe->A * Plan::n));
     FE_CUDA(fe, cudaMalloc(&fe->d_tw2s, sizeof(float2) * (size_t)Plan::R2 * Plan::M2));
     build_scalar_twiddles<<<(Plan::R2 * Plan::M2 + 255) / 256, 256>>>(fe->d_tw2s, Plan::R2, Plan::M2, Plan::M1);
     FE_CUDA(fe, cudaGetLastError());
@@ -359,8 +362,15 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
         xp2.tw1 = fe->d_tw1s;
         xp2.tw2 = fe->d_tw2s;
         xp2.tpost = fe->d_tpost;
-        xp2.rg = fe->d_rg;
-        xp2.gains = fe->d_gains;
+        const int mode = per_spectrum ? 1 : 0;
+        if (fe->rg2_mode != mode) {
+            dim3 grid((unsigned)((fe->n + 255) / 256), (unsigned)fe->A);
+            build_rg2_table<<<grid, 256, 0, stream>>>(fe->d_rg2, fe->d_gains, fe->d_coarse, fe->d_fine_d, fe->d_fine_phi,
+                                                     fe->n, fe->A, mode);
+            fe->rg2_mode = mode;
+            ++fe->last_launches;
+        }
+        xp2.rg2 = fe->d_rg2;
         xp2.coarse = fe->d_coarse;
         xp2.fine_d = fe->d_fine_d;
         xp2.fine_phi = fe->d_fine_phi;
@@ -492,6 +502,7 @@ void fengine_destroy(fengine_t *fe)
     cudaFree(fe->d_tpost);
     cudaFree(fe->d_tw1s);
     cudaFree(fe->d_tw2s);
+    cudaFree(fe->d_rg2);
     cudaFree(fe->d_scratch);
     cudaFree(fe->d_stage_in);
     cudaFree(fe->d_stage_out);
@@ -526,6 +537,7 @@ int fengine_set_coarse_delays(fengine_t *fe, const int32_t *c, int64_t n_per_str
             fe->pols_equal = memcmp(c + (size_t)(2 * a) * n_per_stream, c + (size_t)(2 * a + 1) * n_per_stream,
                                     sizeof(int32_t) * (size_t)n_per_stream) == 0;
     fe->rg_dirty = true;
+    fe->rg2_mode = -1;
     return FENGINE_OK;
 }
 
@@ -554,6 +566,7 @@ int fengine_set_fine_delays(fengine_t *fe, const float *delay, const float *phas
     FE_CUDA(fe, cudaMemcpy(fe->d_fine_d, delay, sizeof(float) * count, cudaMemcpyHostToDevice));
     FE_CUDA(fe, cudaMemcpy(fe->d_fine_phi, phase, sizeof(float) * count, cudaMemcpyHostToDevice));
     fe->rg_dirty = true;
+    fe->rg2_mode = -1;
     return FENGINE_OK;
 }
 
@@ -567,6 +580,7 @@ int fengine_set_gains(fengine_t *fe, const float *gains_re_im)
     FE_CUDA(fe, cudaDeviceSynchronize());
     FE_CUDA(fe, cudaMemcpy(fe->d_gains, gains_re_im, sizeof(float2) * count, cudaMemcpyHostToDevice));
     fe->rg_dirty = true;
+    fe->rg2_mode = -1;
     return FENGINE_OK;
 }
 
