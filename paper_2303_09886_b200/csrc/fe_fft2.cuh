@@ -17,6 +17,10 @@
 #include "fe_common.cuh"
 #include "fe_fft.cuh"
 
+#ifndef FE_TW1_POWERS
+#define FE_TW1_POWERS 1
+#endif
+
 namespace fe {
 
 template <int N_CH, int R2_, int R3_, int TPF>
@@ -64,12 +68,25 @@ __device__ __forceinline__ void fft2_pass1(const float4 *__restrict__ grow, floa
             x[t].im = f2(v.z, v.w);
         }
         Dif<R, f2>::run(x);
+#if FE_TW1_POWERS
+        // W_n^{k col}, k = 1..15, as powers of the one table word W_n^{col} (product tree of depth <= 4: the
+        // rounding error stays below 5e-7, far inside the 1e-4 budget), so pass 1 reads 8 bytes of table per
+        // butterfly instead of 120 and the table never competes with the gain table for the L1
+        float2 w[R];
+        w[1] = __ldg(tw + M1 + col);
+#pragma unroll
+        for (int k = 2; k < R; ++k) w[k] = cmulf(w[k / 2], w[k - k / 2]);
+#endif
 #pragma unroll
         for (int k = 0; k < R; ++k) {
             cx<f2> y = x[k];
             if (k > 0) {
-                const float2 w = __ldg(tw + k * M1 + col);
-                y = cmul(x[k], w.x, w.y);
+#if FE_TW1_POWERS
+                y = cmul(x[k], w[k].x, w[k].y);
+#else
+                const float2 wk = __ldg(tw + k * M1 + col);
+                y = cmul(x[k], wk.x, wk.y);
+#endif
             }
             sm[k * Plan::blk + col] = make_float4(y.re.v.x, y.re.v.y, y.im.v.x, y.im.v.y);
         }
@@ -198,13 +215,27 @@ __device__ __forceinline__ void fft2_pass3(float4 *sm, const Fft2Params &prm, in
         }
         base = {f2(e[0].x, e[1].x), f2(e[0].y, e[1].y)};
     }
-    const float2 *__restrict__ tpost = prm.tpost;
+    // post-twiddle phasors without a table walk: (sin, cos)(2 pi (K + Q kq) / N) = the thread's own (sin, cos)(2 pi K / N)
+    // rotated by the compile-time angle 2 pi kq Q / N (Q / N is 1/32 or 1/16), one table word per thread and spectrum
+    const float2 tpK = __ldg(prm.tpost + K);
+    auto tp_of = [&](int kq) {
+        constexpr int st = 32 * Q / N;
+        const float cphi = w32_cos(kq * st), sphi = w32_sin(kq * st);
+        return make_float2(fmaf(tpK.x, cphi, tpK.y * sphi), fmaf(-tpK.x, sphi, tpK.y * cphi));
+    };
     uint32_t *rec = F32OUT ? nullptr : reinterpret_cast<uint32_t *>(prm.out + (((int64_t)a * prm.n_spectra + m) * n) * 4);
     float4 *yout = F32OUT ? reinterpret_cast<float4 *>(prm.out_f32 + (((int64_t)a * prm.n_spectra + m) * n) * 4) : nullptr;
 
-    auto rot_gain = [&](int kq, int kA, int kB, cx<f2> &rgA, cx<f2> &rgB) {
-        const cx<f2> gA = unpack_unit(__ldg(gtab + kA));
-        const cx<f2> gB = unpack_unit(__ldg(gtab + (kB & (n - 1))));
+    // every gain word of this thread's channels is requested before the exchange barrier so that the L2 latency of
+    // the table overlaps the barrier and the mirror loads instead of being paid once per channel pair
+    float4 gA[H], gB[H];
+#pragma unroll
+    for (int kq = 0; kq < H; ++kq) {
+        const int kA = K + Q * kq;
+        gA[kq] = __ldg(gtab + kA);
+        gB[kq] = __ldg(gtab + ((n - kA) & (n - 1)));
+    }
+    auto rot_gain = [&](int kq, cx<f2> gA_, cx<f2> gB_, cx<f2> &rgA, cx<f2> &rgB) {
         if (prm.per_spectrum) {
             const cx<f2> E = cmul2(base, unpack_unit(sph->step[kq]));
             const cx<f2> Ec = {E.re, -E.im};
@@ -212,30 +243,29 @@ __device__ __forceinline__ void fft2_pass3(float4 *sm, const Fft2Params &prm, in
             const cx<f2> c3 = unpack_unit(sph->c3);
             const cx<f2> eB0 = cmul2(c3, Ec);
             const cx<f2> eB = {eB0.re * 0.5f, eB0.im * 0.5f};
-            rgA = cmul2(eA, gA);
-            rgB = cmul2(eB, gB);
+            rgA = cmul2(eA, gA_);
+            rgB = cmul2(eB, gB_);
         } else {
-            rgA = gA;
-            rgB = gB;
+            rgA = gA_;
+            rgB = gB_;
         }
     };
 
     __syncthreads();                                      // upper halves are in the exchange buffer
-    cx<f2> zm[H];
-#pragma unroll
-    for (int j = 0; j < H; ++j) zm[j] = unpack_unit(theirs[j]);
 #pragma unroll
     for (int kq = 0; kq < H; ++kq) {
         const int kA = K + Q * kq, kB = n - kA;            // kB == n for the DC channel (dropped Nyquist)
+        const cx<f2> zmk = unpack_unit(theirs[kq]);
         cx<f2> rgA, rgB;
-        rot_gain(kq, kA, kB, rgA, rgB);
-        fft2_epilogue<F32OUT>(z[kq], zm[kq], __ldg(tpost + kA), rgA, rgB, kA, kB, n, rec, yout);
+        rot_gain(kq, unpack_unit(gA[kq]), unpack_unit(gB[kq]), rgA, rgB);
+        fft2_epilogue<F32OUT>(z[kq], zmk, kq == 0 ? tpK : tp_of(kq), rgA, rgB, kA, kB, n, rec, yout);
     }
     if (K == 0) {                                         // channel n/2 = Q * H mirrors onto itself
         const cx<f2> zh = unpack_unit(mine[H]);
         cx<f2> rgA, rgB;
-        rot_gain(H, n / 2, n / 2, rgA, rgB);
-        fft2_epilogue<F32OUT>(zh, zh, __ldg(tpost + n / 2), rgA, rgB, n / 2, n, n, rec, yout);
+        const cx<f2> gh = unpack_unit(__ldg(gtab + n / 2));
+        rot_gain(H, gh, gh, rgA, rgB);
+        fft2_epilogue<F32OUT>(zh, zh, make_float2(1.0f, 0.0f), rgA, rgB, n / 2, n, n, rec, yout);
     }
 }
 

@@ -140,6 +140,8 @@ int launch_fft2(fengine *fe, const Fft2Params &prm, int64_t chunk_len, cudaStrea
     static bool attr_set = false;
     if (!attr_set) {
         FE_CUDA(fe, cudaFuncSetAttribute(fft2_kernel<Plan, F32OUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        if (const char *cv = getenv("FE_FFT2_CARVEOUT"))
+            FE_CUDA(fe, cudaFuncSetAttribute(fft2_kernel<Plan, F32OUT>, cudaFuncAttributePreferredSharedMemoryCarveout, atoi(cv)));
         attr_set = true;
     }
     dim3 grid((unsigned)chunk_len, (unsigned)fe->A);
