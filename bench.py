@@ -147,6 +147,7 @@ def main():
     ap.add_argument("--n-spectra", type=int, default=None, help="shrink the batch (debugging only)")
     ap.add_argument("--chunk-spectra", type=int, default=None)
     ap.add_argument("--fir-rows", type=int, default=None)
+    ap.add_argument("--opt", action="append", default=[], help="library option key=value (fengine_set_option), repeatable")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -179,6 +180,9 @@ def main():
         fe.set_option("chunk_spectra", args.chunk_spectra)
     if args.fir_rows is not None:
         fe.set_option("fir_rows", args.fir_rows)
+    for kv in args.opt:
+        k, v = kv.split("=")
+        fe.set_option(k, int(v))
 
     host_in = torch.from_numpy(w.packed.reshape(-1))
     in_bytes, out_shape = host_in.numel(), fe.output_shape(w.S)

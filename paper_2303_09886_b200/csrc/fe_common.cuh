@@ -62,23 +62,37 @@ __device__ __forceinline__ cx<V> cmul(cx<V> a, W wr, W wi)
 template <typename V>
 __device__ __forceinline__ cx<V> mul_neg_i(cx<V> a) { return {a.im, -a.re}; }
 
-// streaming global accesses that should not displace the L1-resident tables
+// streaming global accesses that should not displace the L1-resident tables.  The scratch rows are read at L2
+// (ld.global.cg): they were written by another CTA (of an earlier kernel, or of the same fused kernel after a
+// release / acquire handshake) and a ring slot's addresses are reused, so the L1 must never serve them.
 __device__ __forceinline__ float4 ldg_stream_f4(const float4 *p)
 {
     float4 v;
-    asm volatile("ld.global.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
+    asm volatile("ld.global.cg.v4.f32 {%0,%1,%2,%3}, [%4];"
                  : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
     return v;
 }
 __device__ __forceinline__ void stg_stream_f4(float4 *p, float4 v)
 {
-    asm volatile("st.global.L1::no_allocate.v4.f32 [%0], {%1,%2,%3,%4};"
+    asm volatile("st.global.cg.v4.f32 [%0], {%1,%2,%3,%4};"
                  :: "l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
 }
 __device__ __forceinline__ void stg_stream_u4(uint4 *p, uint4 v)
 {
     asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};"
                  :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+// release / acquire handshake on a device-scope counter (fused kernel: FIR tasks -> FFT tasks -> ring slot reuse)
+__device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int *p)
+{
+    unsigned int v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void red_release_add_u32(unsigned int *p, unsigned int v)
+{
+    asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
 // floor division / modulus by a positive power of two given as log2

@@ -269,6 +269,62 @@ __device__ __forceinline__ void fft2_pass3(float4 *sm, const Fft2Params &prm, in
     }
 }
 
+// Per-spectrum phasor setup (per-spectrum mode only): warp p sets up pol p's phasors in shared memory.
+template <class Plan>
+__device__ __forceinline__ void fft2_setup_phase(const Fft2Params &prm, SpectrumPhase2 *sph, int a, int64_t m, int tid)
+{
+    constexpr int N = 2 * Plan::n;
+    const int p = tid >> 5, t = tid & 31;
+    if (p < 2 && t <= 16) {
+        const int64_t st = (int64_t)a * 2 + p;
+        const int32_t c = prm.coarse[st * prm.n_coarse + (prm.n_coarse == 1 ? 0 : m)];
+        const int cr = (int)(c & (N - 1));
+        const double d = (double)prm.fine_d[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
+        const double phi = (double)prm.fine_phi[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
+        if (t < 16) {
+            const int k = Plan::Q * t;
+            const double tt = -(d / (double)N) * (double)k - (double)((cr * k) & (N - 1)) / (double)N;
+            const float2 v = phasor_turns(tt);
+            float *dst = reinterpret_cast<float *>(&sph->step[t]);
+            dst[p] = v.x;
+            dst[2 + p] = v.y;
+        } else {
+            double s, c_;
+            sincos(phi, &s, &c_);
+            float *de = reinterpret_cast<float *>(&sph->ephi);
+            de[p] = (float)c_;
+            de[2 + p] = (float)s;
+            sincos(2.0 * phi, &s, &c_);
+            const float2 e2 = make_float2((float)c_, (float)s);
+            float2 h = phasor_turns(-0.5 * d);        // exp(-i pi d_eff) = exp(-i pi d) * (-1)^cr
+            if (cr & 1) { h.x = -h.x; h.y = -h.y; }
+            const float2 c3 = cmulf(e2, h);
+            float *dc = reinterpret_cast<float *>(&sph->c3);
+            dc[p] = c3.x;
+            dc[2 + p] = c3.y;
+        }
+    }
+}
+
+// One spectrum of one antenna, both pols, by the whole CTA.  `after_load()` runs (on every thread) once the
+// scratch row has been consumed (after the barrier that ends pass 1); the fused kernel releases the ring slot there.
+// `after_pass2()` runs after the barrier that ends pass 2 (the fused kernel samples its next task's dependency there).
+template <class Plan, bool F32OUT, class AfterLoad, class AfterPass2>
+__device__ __forceinline__ void fft2_row(const Fft2Params &prm, const float4 *grow, unsigned char *smem_raw, int a,
+                                         int64_t m, int tid, AfterLoad after_load, AfterPass2 after_pass2)
+{
+    float4 *sm = reinterpret_cast<float4 *>(smem_raw);
+    SpectrumPhase2 *sph = reinterpret_cast<SpectrumPhase2 *>(smem_raw + (size_t)Plan::units * 16);
+    if (prm.per_spectrum) fft2_setup_phase<Plan>(prm, sph, a, m, tid);
+    fft2_pass1<Plan>(grow, sm, prm.tw1, tid);
+    __syncthreads();
+    after_load();
+    fft2_pass2<Plan>(sm, prm.tw2, tid);
+    __syncthreads();
+    after_pass2();
+    fft2_pass3<Plan, F32OUT>(sm, prm, a, m, tid, sph);
+}
+
 template <class Plan>
 constexpr size_t fft2_smem_bytes()
 {
@@ -280,55 +336,12 @@ template <class Plan, bool F32OUT>
 __global__ void __launch_bounds__(Plan::tpf, (512 / Plan::tpf) > 0 ? (512 / Plan::tpf) : 1) fft2_kernel(const Fft2Params prm)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    constexpr int n = Plan::n, N = 2 * n;
-    float4 *sm = reinterpret_cast<float4 *>(smem_raw);
-    SpectrumPhase2 *sph = reinterpret_cast<SpectrumPhase2 *>(smem_raw + (size_t)Plan::units * 16);
-
-    const int tid = threadIdx.x;
+    constexpr int N = 2 * Plan::n;
     const int a = blockIdx.y;
     const int64_t m = prm.m_begin + blockIdx.x;
     if (m >= prm.m_end) return;
-
     const float4 *grow = reinterpret_cast<const float4 *>(prm.g + ((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * (int64_t)N * 2);
-
-    if (prm.per_spectrum) {                               // warp p sets up pol p's phasors
-        const int p = tid >> 5, t = tid & 31;
-        if (p < 2 && t <= 16) {
-            const int64_t st = (int64_t)a * 2 + p;
-            const int32_t c = prm.coarse[st * prm.n_coarse + (prm.n_coarse == 1 ? 0 : m)];
-            const int cr = (int)(c & (N - 1));
-            const double d = (double)prm.fine_d[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
-            const double phi = (double)prm.fine_phi[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
-            if (t < 16) {
-                const int k = Plan::Q * t;
-                const double tt = -(d / (double)N) * (double)k - (double)((cr * k) & (N - 1)) / (double)N;
-                const float2 v = phasor_turns(tt);
-                float *dst = reinterpret_cast<float *>(&sph->step[t]);
-                dst[p] = v.x;
-                dst[2 + p] = v.y;
-            } else {
-                double s, c_;
-                sincos(phi, &s, &c_);
-                float *de = reinterpret_cast<float *>(&sph->ephi);
-                de[p] = (float)c_;
-                de[2 + p] = (float)s;
-                sincos(2.0 * phi, &s, &c_);
-                const float2 e2 = make_float2((float)c_, (float)s);
-                float2 h = phasor_turns(-0.5 * d);        // exp(-i pi d_eff) = exp(-i pi d) * (-1)^cr
-                if (cr & 1) { h.x = -h.x; h.y = -h.y; }
-                const float2 c3 = cmulf(e2, h);
-                float *dc = reinterpret_cast<float *>(&sph->c3);
-                dc[p] = c3.x;
-                dc[2 + p] = c3.y;
-            }
-        }
-    }
-
-    fft2_pass1<Plan>(grow, sm, prm.tw1, tid);
-    __syncthreads();
-    fft2_pass2<Plan>(sm, prm.tw2, tid);
-    __syncthreads();
-    fft2_pass3<Plan, F32OUT>(sm, prm, a, m, tid, sph);
+    fft2_row<Plan, F32OUT>(prm, grow, smem_raw, a, m, threadIdx.x, [] {}, [] {});
 }
 
 // Pol-interleaved table of the pol-packed epilogue, [A][n] units {re p0, re p1, im p0, im p1}:

@@ -21,6 +21,7 @@
 #include "fe_fft2.cuh"
 #include "fe_fir.cuh"
 #include "fe_fir2.cuh"
+#include "fe_fused.cuh"
 #include "fe_generic.cuh"
 
 using namespace fe;
@@ -45,6 +46,16 @@ struct fengine {
     // scratch
     float *d_scratch = nullptr;
     size_t scratch_floats = 0;
+    // fused kernel (fe_fused.cuh): L2-resident ring of scratch slots and its control words
+    float *d_ring = nullptr;
+    size_t ring_floats = 0;
+    unsigned int *d_ctl = nullptr;
+    size_t ctl_words = 0;
+    bool allow_fused = false;       // option "fused" (off by default: see DESIGN.md section 6)
+    int ring_slots = 8;             // option "ring_slots" (D)
+    int lag = 5;                    // option "lag" (phases between a unit's FIR and FFT tasks)
+    int fused_ctas_per_sm = 0;      // option "fused_ctas_per_sm" (0 = occupancy)
+    int n_sms = 0;
     bool rg_dirty = true;
     // staging for fengine_process_host
     uint8_t *d_stage_in = nullptr;
@@ -158,6 +169,86 @@ int launch_fft2_n(fengine *fe, const Fft2Params &prm, int64_t chunk_len, cudaStr
     case 4096: return launch_fft2<Plan2_4096, F32OUT>(fe, prm, chunk_len, stream);
     }
     return fail(fe, FENGINE_ERR_INVALID_ARG, "no pol-packed FFT plan for n=%d", fe->n);
+}
+
+bool use_fused(const fengine *fe) { return use_packed(fe) && fe->allow_fused && (fe->T == 4 || fe->T == 8 || fe->T == 16); }
+
+template <int T, class Plan, bool F32OUT>
+int launch_fused(fengine *fe, const FusedParams &prm, cudaStream_t stream)
+{
+    const size_t smem = fft2_smem_bytes<Plan>();
+    static int ctas_per_sm = 0;
+    if (!ctas_per_sm) {
+        FE_CUDA(fe, cudaFuncSetAttribute(fused2_kernel<T, Plan, F32OUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        FE_CUDA(fe, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, fused2_kernel<T, Plan, F32OUT>, Plan::tpf, smem));
+        if (getenv("FE_DEBUG")) fprintf(stderr, "fused2_kernel: occupancy %d CTAs/SM, smem %zu\n", ctas_per_sm, smem);
+        if (ctas_per_sm < 1) ctas_per_sm = 1;
+    }
+    const int per_sm = fe->fused_ctas_per_sm > 0 ? fe->fused_ctas_per_sm : ctas_per_sm;
+    // never more CTAs than tasks: a CTA that finds no ticket exits at once, but it still costs a launch slot
+    const int64_t tasks = (int64_t)prm.U * (prm.nb + prm.C);
+    const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>((int64_t)per_sm * fe->n_sms, tasks));
+    fused2_kernel<T, Plan, F32OUT><<<grid, Plan::tpf, smem, stream>>>(prm);
+    return FENGINE_OK;
+}
+
+template <int T, bool F32OUT>
+int launch_fused_n(fengine *fe, const FusedParams &prm, cudaStream_t stream)
+{
+    switch (fe->n) {
+    case 1024: return launch_fused<T, Plan2_1024, F32OUT>(fe, prm, stream);
+    case 2048: return launch_fused<T, Plan2_2048, F32OUT>(fe, prm, stream);
+    case 4096: return launch_fused<T, Plan2_4096, F32OUT>(fe, prm, stream);
+    }
+    return fail(fe, FENGINE_ERR_INVALID_ARG, "no fused plan for n=%d", fe->n);
+}
+
+template <bool F32OUT>
+int launch_fused_T(fengine *fe, const FusedParams &prm, cudaStream_t stream)
+{
+    switch (fe->T) {
+    case 4: return launch_fused_n<4, F32OUT>(fe, prm, stream);
+    case 8: return launch_fused_n<8, F32OUT>(fe, prm, stream);
+    case 16: return launch_fused_n<16, F32OUT>(fe, prm, stream);
+    }
+    return fail(fe, FENGINE_ERR_INVALID_ARG, "no fused kernel for T=%d", fe->T);
+}
+
+int tpf_of(int n) { return n == 4096 ? Plan2_4096::tpf : n == 2048 ? Plan2_2048::tpf : Plan2_1024::tpf; }
+
+// ring and control words of the fused kernel for a call of S spectra
+int ensure_fused(fengine *fe, int64_t S, int C, int D)
+{
+    const size_t floats = (size_t)D * C * fe->N * 2;
+    if (floats > fe->ring_floats) {
+        if (fe->d_ring) {
+            FE_CUDA(fe, cudaDeviceSynchronize());
+            cudaFree(fe->d_ring);
+            fe->d_ring = nullptr;
+            fe->ring_floats = 0;
+        }
+        if (cudaMalloc(&fe->d_ring, floats * sizeof(float)) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(fe, FENGINE_ERR_ALLOC, "cannot allocate %zu bytes of ring", floats * sizeof(float));
+        }
+        fe->ring_floats = floats;
+    }
+    const size_t U = (size_t)((S + C - 1) / C) * fe->A;
+    const size_t words = 4 + 2 * U;
+    if (words > fe->ctl_words) {
+        if (fe->d_ctl) {
+            FE_CUDA(fe, cudaDeviceSynchronize());
+            cudaFree(fe->d_ctl);
+            fe->d_ctl = nullptr;
+            fe->ctl_words = 0;
+        }
+        if (cudaMalloc(&fe->d_ctl, words * sizeof(unsigned int)) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(fe, FENGINE_ERR_ALLOC, "cannot allocate the control words of the fused kernel");
+        }
+        fe->ctl_words = words;
+    }
+    return FENGINE_OK;
 }
 
 int launch_fir2(fengine *fe, const Fir2Params &prm, int64_t chunk_len, cudaStream_t stream)
@@ -308,7 +399,8 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
     }
 
     const int64_t chunk = fe->chunk_spectra > 0 ? std::min<int64_t>(fe->chunk_spectra, S) : S;
-    int rc = ensure_scratch(fe, (size_t)streams * chunk * fe->N);
+    const bool fused = use_fused(fe);
+    int rc = fused ? FENGINE_OK : ensure_scratch(fe, (size_t)streams * chunk * fe->N);
     if (rc) return rc;
 
     FirParams fp{};
@@ -383,6 +475,48 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
         xp2.per_spectrum = per_spectrum ? 1 : 0;
     }
 
+    if (fused) {
+        const int C = (int)std::min<int64_t>(fe->fir_rows, S);
+        const int LAG = fe->lag, D = std::max(fe->ring_slots, LAG + 2);
+        rc = ensure_fused(fe, S, C, D);
+        if (rc) return rc;
+        FusedParams up{};
+        up.fir = fp2;
+        up.fft = xp2;
+        up.fir.m_begin = up.fft.m_begin = 0;
+        up.fir.m_end = up.fft.m_end = S;
+        up.ring = fe->d_ring;
+        up.ctl = fe->d_ctl;
+        up.S = S;
+        up.A = fe->A;
+        up.C = C;
+        up.D = D;
+        up.LAG = LAG;
+        up.U = (int)((S + C - 1) / C) * fe->A;
+        up.nb = fe->n / tpf_of(fe->n);
+        cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+        if (fe->profile) {
+            for (auto &e : ev) {
+                if (fe->ev_pool.empty()) {
+                    FE_CUDA(fe, cudaEventCreate(&e));
+                } else {
+                    e = fe->ev_pool.back();
+                    fe->ev_pool.pop_back();
+                }
+                fe->ev_used.push_back(e);
+            }
+            FE_CUDA(fe, cudaEventRecord(ev[0], stream));
+            FE_CUDA(fe, cudaEventRecord(ev[1], stream));    // no separate FIR launch: the whole step is the fused kernel
+        }
+        FE_CUDA(fe, cudaMemsetAsync(fe->d_ctl, 0, sizeof(unsigned int) * (4 + 2 * (size_t)up.U), stream));
+        rc = out_f32 ? launch_fused_T<true>(fe, up, stream) : launch_fused_T<false>(fe, up, stream);
+        if (rc) return rc;
+        if (fe->profile) FE_CUDA(fe, cudaEventRecord(ev[2], stream));
+        fe->last_launches += 1;
+        FE_CUDA(fe, cudaGetLastError());
+        return FENGINE_OK;
+    }
+
     for (int64_t m0 = 0; m0 < S; m0 += chunk) {
         const int64_t m1 = std::min(S, m0 + chunk);
         fp.m_begin = xp.m_begin = fp2.m_begin = xp2.m_begin = m0;
@@ -441,6 +575,12 @@ fengine_t *fengine_create_batched(int n_antennas, int n_channels, int taps, int 
     while ((1 << fe->lgN) < N) ++fe->lgN;
     fe->tiled = tiled_n(fe->n) && tiled_T(fe->T);
     const size_t streams = (size_t)fe->A * fe->P;
+    {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&fe->n_sms, cudaDevAttrMultiProcessorCount, dev);
+        if (fe->n_sms < 1) fe->n_sms = 148;
+    }
 
     bool ok = cudaMalloc(&fe->d_weights, sizeof(float) * (size_t)N * taps) == cudaSuccess &&
               cudaMalloc(&fe->d_coarse, sizeof(int32_t) * streams) == cudaSuccess &&
@@ -506,6 +646,8 @@ void fengine_destroy(fengine_t *fe)
     cudaFree(fe->d_tw2s);
     cudaFree(fe->d_rg2);
     cudaFree(fe->d_scratch);
+    cudaFree(fe->d_ring);
+    cudaFree(fe->d_ctl);
     cudaFree(fe->d_stage_in);
     cudaFree(fe->d_stage_out);
     if (fe->host_stream) cudaStreamDestroy(fe->host_stream);
@@ -727,6 +869,25 @@ int fengine_set_option(fengine_t *fe, const char *key, int64_t value)
     }
     if (!strcmp(key, "pol_packed")) {
         fe->allow_packed = value != 0;
+        return FENGINE_OK;
+    }
+    if (!strcmp(key, "fused")) {
+        fe->allow_fused = value != 0;
+        return FENGINE_OK;
+    }
+    if (!strcmp(key, "ring_slots")) {
+        if (value < 2 || value > 1024) return fail(fe, FENGINE_ERR_INVALID_ARG, "ring_slots out of range");
+        fe->ring_slots = (int)value;
+        return FENGINE_OK;
+    }
+    if (!strcmp(key, "lag")) {
+        if (value < 1 || value > 1022) return fail(fe, FENGINE_ERR_INVALID_ARG, "lag out of range");
+        fe->lag = (int)value;
+        return FENGINE_OK;
+    }
+    if (!strcmp(key, "fused_ctas_per_sm")) {
+        if (value < 0 || value > 32) return fail(fe, FENGINE_ERR_INVALID_ARG, "fused_ctas_per_sm out of range");
+        fe->fused_ctas_per_sm = (int)value;
         return FENGINE_OK;
     }
     if (!strcmp(key, "force_generic")) {
