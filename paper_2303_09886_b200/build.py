@@ -46,6 +46,16 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     return LIB
 
 
+def build_tools() -> Path:
+    """The FP32 issue-rate microbenchmark (csrc/fp32_rate.cu), a standalone program."""
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    exe = PKG / "fp32_rate"
+    subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", str(exe), str(CSRC / "fp32_rate.cu")])
+    return exe
+
+
 if __name__ == "__main__":
     build(force="--force" in sys.argv, verbose="-v" in sys.argv)
     print(LIB)
+    if "--tools" in sys.argv:
+        print(build_tools())
