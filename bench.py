@@ -225,12 +225,10 @@ def main():
     torch.cuda.synchronize()
     clocks = sampler.stop()
 
-    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total = float(t.item())
+    from paper_2303_09886_b200 import sharding
+    ms_total = sharding.max_over_ranks(ms_total, dist if world > 1 else None, device="cuda")
     ms_per_step = ms_total / args.steps
-    value = world * units_per_step / (ms_per_step * 1e-3) / 1e9
+    value = sharding.aggregate_rate(units_per_step, world, ms_per_step * 1e-3) / 1e9
 
     # ---- per-kernel durations (CUDA events recorded by the library on the launching stream) ----
     fe.set_option("profile", 1)
@@ -255,6 +253,20 @@ def main():
         "note": "achieved = 4.5 B per dual-pol sample x samples per launch / dominant kernel's mean duration; "
                 "step_frac is the same bytes over the whole step (the metric's % of HBM roofline)",
     }
+    # The path is bound by the plain FP32 pipe before it is bound by HBM:
+    # north-star accounting, FIR 2T flop + FFT 5 n log2(n) / N flop per real sample; an FMA is one lane-operation
+    # (2 flop), the FFT's adds and multiplies are one lane-operation each.  Peak = measured packed-FP32 issue rate
+    # (profiles/r1_fp32_rate.txt: 125.5 lane-ops/clk/SM x 148 SMs x 1.965 GHz).
+    lane_ops_per_real = w.T + 5.0 * w.n * np.log2(w.n) / w.N
+    alu_peak = 125.5 * 148 * 1.965e9
+    alu_achieved = lane_ops_per_real * w.P * units_per_step / (ms_per_step * 1e-3)
+    roofline["alu"] = {"bound": "alu", "achieved": alu_achieved / 1e12, "peak": alu_peak / 1e12, "unit": "T lane-op/s",
+                       "frac": alu_achieved / alu_peak, "lane_ops_per_real_sample": lane_ops_per_real,
+                       "note": "whole step against the measured FP32 issue rate; the slower of this and the HBM roofline "
+                               "is the north star's roofline"}
+    roofline["fused"] = bool(n_fir and fir_avg < 0.02 * max(fft_avg, 1e-9))
+    if roofline["fused"]:
+        roofline["kernel"] = dom_name = "fused_kernel"
     prof = ROOT / "profiles" / "roofline_traffic.json"
     if prof.exists():
         try:

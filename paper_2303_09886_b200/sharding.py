@@ -1,0 +1,27 @@
+"""Multi-GPU layout of the path: antennas are independent, so they shard across ranks with the
+weights replicated and no data-path collective.  Host logic only."""
+from __future__ import annotations
+
+
+def shard_antennas(n_antennas: int, world: int, rank: int) -> range:
+    """Contiguous block of antennas owned by `rank`; blocks differ in size by at most one."""
+    if world < 1 or not (0 <= rank < world) or n_antennas < 0:
+        raise ValueError("bad shard request")
+    base, extra = divmod(n_antennas, world)
+    start = rank * base + min(rank, extra)
+    return range(start, start + base + (1 if rank < extra else 0))
+
+
+def max_over_ranks(value: float, dist=None, device=None) -> float:
+    """Max of a timing scalar over the ranks of the default process group (the only collective of the job)."""
+    if dist is None or not dist.is_available() or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(value)
+    import torch
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_rate(units_per_rank: int, world: int, seconds_max: float) -> float:
+    """Whole-job throughput: units all ranks processed / slowest rank's time (weak scaling)."""
+    return world * units_per_rank / seconds_max
