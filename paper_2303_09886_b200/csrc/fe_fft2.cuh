@@ -17,6 +17,9 @@
 #include "fe_common.cuh"
 #include "fe_fft.cuh"
 
+#ifndef FE_FFT2_MINB
+#define FE_FFT2_MINB 2
+#endif
 #ifndef FE_TW1_POWERS
 #define FE_TW1_POWERS 1
 #endif
@@ -333,7 +336,7 @@ constexpr size_t fft2_smem_bytes()
 
 // One CTA per (antenna, spectrum), both pols.
 template <class Plan, bool F32OUT>
-__global__ void __launch_bounds__(Plan::tpf, (512 / Plan::tpf) > 0 ? (512 / Plan::tpf) : 1) fft2_kernel(const Fft2Params prm)
+__global__ void __launch_bounds__(Plan::tpf, FE_FFT2_MINB * ((512 / Plan::tpf) > 0 ? (512 / Plan::tpf) : 1) / 2) fft2_kernel(const Fft2Params prm)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int N = 2 * Plan::n;

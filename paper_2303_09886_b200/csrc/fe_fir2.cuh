@@ -121,22 +121,35 @@ __device__ __forceinline__ void fir2_run(const Fir2Params &prm, const uint8_t *w
     float *gp = grow0 + 4 * i_pt + ((int64_t)(MIXED ? 0 : lag0) - T) * (int64_t)g_stride;
     int sp = (MIXED ? 0 : lag0) - T;
 
+    // The loop is software-pipelined by one step and has no branch in its unrolled body: the raw words of step
+    // ii + 1 are read from the ring while the FMAs of step ii issue, and the scratch store is a predicated
+    // instruction, so the unpack chain (LDS -> PRMT -> SHF -> I2FP) of the next step hides behind 32 FFMA2s.
+    auto load_raw = [&](int slot, uint32_t (&raw)[4]) {
+        const uint32_t ad = rd_addr + slot * kFir2SlotBytes;
+        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(raw[0]) : "r"(ad) : "memory");
+        asm volatile("ld.shared.u32 %0, [%1+4];" : "=r"(raw[1]) : "r"(ad) : "memory");
+        asm volatile("ld.shared.u32 %0, [%1+80];" : "=r"(raw[2]) : "r"(ad) : "memory");
+        asm volatile("ld.shared.u32 %0, [%1+84];" : "=r"(raw[3]) : "r"(ad) : "memory");
+    };
+    uint32_t nxt[4];
+    cp_async_wait<kFirRingBatches - 2>();
+    __syncwarp();
+    issue_batch((kFirRingBatches - 1) * kFirBatch);
+    load_raw(0, nxt);
+
     const int n_steps = n_out + T;
     for (int i0 = 0; i0 < n_steps; i0 += U) {
 #pragma unroll
         for (int ii = 0; ii < U; ++ii) {
-            if (ii % kFirBatch == 0) {
+            const uint32_t P0a = nxt[0], P0b = nxt[1], P1a = nxt[2], P1b = nxt[3];
+            if ((ii + 1) % kFirBatch == 0) {
+                // the batch that holds step ii + 1 has landed; every lane holds the words of step ii, so the batch
+                // issued now may overwrite the slots of steps ii - 3 .. ii
                 cp_async_wait<kFirRingBatches - 2>();
                 __syncwarp();
-                issue_batch(((ii / kFirBatch + kFirRingBatches - 1) % kFirRingBatches) * kFirBatch);
+                issue_batch((((ii + 1) / kFirBatch + kFirRingBatches - 1) % kFirRingBatches) * kFirBatch);
             }
-            const int slot = ii % kFirDepth;
-            uint32_t P0a, P0b, P1a, P1b;
-            const uint32_t ad = rd_addr + slot * kFir2SlotBytes;
-            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(P0a) : "r"(ad) : "memory");
-            asm volatile("ld.shared.u32 %0, [%1+4];" : "=r"(P0b) : "r"(ad) : "memory");
-            asm volatile("ld.shared.u32 %0, [%1+80];" : "=r"(P1a) : "r"(ad) : "memory");
-            asm volatile("ld.shared.u32 %0, [%1+84];" : "=r"(P1b) : "r"(ad) : "memory");
+            load_raw((ii + 1) % kFirDepth, nxt);
             const uint32_t be0 = __byte_perm(P0a, P0b, sel) << sha;     // sample a in bits 31..22, b in 21..12
             const uint32_t be1 = __byte_perm(P1a, P1b, sel) << sha;
             const f2 s0((float)((int32_t)be0 >> 22), (float)((int32_t)be1 >> 22));                  // column v0, (p0, p1)
@@ -160,7 +173,8 @@ __device__ __forceinline__ void fir2_run(const Fir2Params &prm, const uint8_t *w
                 cur.w = lagc[1] ? prev.w : now.w;
                 prev = now;
             }
-            if ((unsigned)sp < (unsigned)n_out) *reinterpret_cast<float4 *>(gp) = cur;
+            asm volatile("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %5, %6;\n\t@p st.global.v4.f32 [%0], {%1, %2, %3, %4};\n\t}"
+                         ::"l"(gp), "f"(cur.x), "f"(cur.y), "f"(cur.z), "f"(cur.w), "r"((unsigned)sp), "r"((unsigned)n_out) : "memory");
             gp += g_stride;
             ++sp;
         }
