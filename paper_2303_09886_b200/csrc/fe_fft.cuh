@@ -162,6 +162,19 @@ struct FftParams {
 };
 
 // ---- pass 1: global (scratch g') -> butterfly -> twiddle -> shared ---------------------------------
+// Pass twiddles W^{k x}, k = 1..R-1, as running powers of the one table word W^{x} (both packed lanes hold their own
+// x): the table walk of R-1 float4 words per butterfly (64 KB per spectrum in pass 1 of n = 8192) becomes one word,
+// which keeps the L1 for the gain table.  The running product adds at most R rounding steps (< 2e-6 relative).
+__device__ __forceinline__ cx<f2> cmulp(cx<f2> a, cx<f2> b)
+{
+    return {fnma_(a.im, b.im, a.re * b.re), fma_(a.im, b.re, a.re * b.im)};
+}
+__device__ __forceinline__ cx<f2> load_tw(const float4 *__restrict__ p)
+{
+    const float4 w = __ldg(p);
+    return {f2(w.x, w.y), f2(w.z, w.w)};
+}
+
 template <class Plan>
 __device__ __forceinline__ void fft_pass_first(const float4 *__restrict__ grow, float4 *sm, const float4 *__restrict__ tw,
                                                int tid)
@@ -176,13 +189,15 @@ __device__ __forceinline__ void fft_pass_first(const float4 *__restrict__ grow, 
             x[t].re = f2(v.x, v.y);
             x[t].im = f2(v.z, v.w);
         }
+        const cx<f2> w1 = load_tw(tw + ncol + col);
         Dif<R, f2>::run(x);
+        cx<f2> wk = w1;
 #pragma unroll
         for (int k = 0; k < R; ++k) {
             cx<f2> y = x[k];
             if (k > 0) {
-                const float4 w = __ldg(tw + k * ncol + col);
-                y = cmul(x[k], f2(w.x, w.y), f2(w.z, w.w));
+                y = cmulp(x[k], wk);
+                if (k + 1 < R) wk = cmulp(wk, w1);
             }
             sm[swz<Plan>(k * ncol + col)] = make_float4(y.re.v.x, y.re.v.y, y.im.v.x, y.im.v.y);
         }
@@ -218,15 +233,18 @@ __device__ __forceinline__ void fft_pass_first_sweep(const float4 *__restrict__ 
     constexpr int ncol = Plan::S(1);
     for (int col = tid; col < ncol; col += Plan::tpf) {
         cx<f2> a[RH];
+        const cx<f2> w1 = load_tw(tw + ncol + col);        // W^{x}; outputs need W^{(2 kk + H) x}
         sweep_half<Plan, H, 0>(grow, col, a);
         Dif<RH, f2>::run(a);
+        const cx<f2> w2 = cmulp(w1, w1);
+        cx<f2> wk = H ? w1 : w2;                           // first non-trivial twiddle: k1 = 1 (H = 1) or 2 (H = 0)
 #pragma unroll
         for (int kk = 0; kk < RH; ++kk) {
             const int k1 = 2 * kk + H;
             cx<f2> y = a[kk];
             if (k1 > 0) {
-                const float4 w = __ldg(tw + k1 * ncol + col);
-                y = cmul(a[kk], f2(w.x, w.y), f2(w.z, w.w));
+                y = cmulp(a[kk], wk);
+                if (kk + 1 < RH) wk = cmulp(wk, w2);
             }
             sm[swz<Plan>(kk * ncol + col)] = make_float4(y.re.v.x, y.re.v.y, y.im.v.x, y.im.v.y);
         }
@@ -250,13 +268,15 @@ __device__ __forceinline__ void fft_pass_mid(float4 *sm, const float4 *__restric
             x[t].re = f2(v.x, v.y);
             x[t].im = f2(v.z, v.w);
         }
+        const cx<f2> w1 = load_tw(tw + Sp + lo);
         Dif<R, f2>::run(x);
+        cx<f2> wk = w1;
 #pragma unroll
         for (int k = 0; k < R; ++k) {
             cx<f2> y = x[k];
             if (k > 0) {
-                const float4 w = __ldg(tw + k * Sp + lo);
-                y = cmul(x[k], f2(w.x, w.y), f2(w.z, w.w));
+                y = cmulp(x[k], wk);
+                if (k + 1 < R) wk = cmulp(wk, w1);
             }
             sm[swz<Plan>(base + k * Sp)] = make_float4(y.re.v.x, y.re.v.y, y.im.v.x, y.im.v.y);
         }
@@ -368,12 +388,34 @@ __device__ __forceinline__ void fft_pass_last(const float4 *sm, const FftParams 
             if (special) base2 = E_of(Q / 2);
         }
 
+        // Table words are requested a group of GK channel pairs ahead of their use (one exposed L2 round trip per
+        // group instead of one per pair), and the post-twiddle phasor of pair kq is the thread's own
+        // (sin, cos)(2 pi K / N) rotated by the compile-time angle 2 pi kq Q / N = 2 pi kq / (2 Rq).
+        constexpr int GK = 4;
+        const float2 tpK = __ldg(tpost + pidx);
+        float2 gAq[GK], gBq[GK];
+        auto k_of = [&](int kq) { return special ? (kq < Rq / 2 ? Q * kq : Q / 2 + Q * (kq - Rq / 2)) : pidx + Q * kq; };
 #pragma unroll
         for (int kq = 0; kq < Rq; ++kq) {
-            const int kA = special ? (kq < Rq / 2 ? Q * kq : Q / 2 + Q * (kq - Rq / 2)) : pidx + Q * kq;
+            if (kq % GK == 0) {
+#pragma unroll
+                for (int g = 0; g < GK; ++g) {
+                    const int kAg = k_of(kq + g);
+                    gAq[g] = __ldg(gtab + kAg);
+                    gBq[g] = __ldg(gtab + ((n - kAg) & (n - 1)));
+                }
+            }
+            const int kA = k_of(kq);
             const int kB = n - kA;                        // == n for the DC pair (dropped Nyquist)
             const cx<float> zk = zA[kq], zm = zB[Rq - 1 - kq];
-            const float2 tp = __ldg(tpost + kA);          // i w^k = (sin, cos)(2 pi k / N)
+            float2 tp;                                    // i w^k = (sin, cos)(2 pi k / N)
+            if (special) {
+                tp = __ldg(tpost + kA);
+            } else {
+                constexpr int st = 32 / (2 * Rq);
+                const float cphi = w32_cos(kq * st), sphi = w32_sin(kq * st);
+                tp = make_float2(fmaf(tpK.x, cphi, tpK.y * sphi), fmaf(-tpK.x, sphi, tpK.y * cphi));
+            }
             const float sr = zk.re + zm.re, si = zk.im - zm.im;     // S = Z[k] + conj Z[n-k]
             const float dr = zk.re - zm.re, di = zk.im + zm.im;     // D = Z[k] - conj Z[n-k]
             const float fr = fmaf(-di, tp.y, dr * tp.x);            // F = D * (i w^k)
@@ -385,14 +427,14 @@ __device__ __forceinline__ void fft_pass_last(const float4 *sm, const FftParams 
                 const bool hi = special && kq >= Rq / 2;
                 const float2 stp = sph->step[hi ? kq - Rq / 2 : kq];
                 const float2 E = cmulf(hi ? base2 : base, stp);
-                const float2 gA = __ldg(gtab + kA);
-                const float2 gB = __ldg(gtab + (kB & (n - 1)));
+                const float2 gA = gAq[kq % GK];
+                const float2 gB = gBq[kq % GK];
                 rgA = cmulf(E, gA);
                 rgB = cmulf(cmulf(sph->c3, make_float2(E.x, -E.y)), gB);
                 rgA.x *= 0.5f; rgA.y *= 0.5f; rgB.x *= 0.5f; rgB.y *= 0.5f;
             } else {
-                rgA = __ldg(gtab + kA);
-                rgB = __ldg(gtab + (kB & (n - 1)));
+                rgA = gAq[kq % GK];
+                rgB = gBq[kq % GK];
             }
             const float yAr = fmaf(-xki, rgA.y, xkr * rgA.x), yAi = fmaf(xki, rgA.x, xkr * rgA.y);
             const float yBr = fmaf(-xmi, rgB.y, xmr * rgB.x), yBi = fmaf(xmi, rgB.x, xmr * rgB.y);

@@ -235,8 +235,8 @@ __device__ __forceinline__ void fft2_pass3(float4 *sm, const Fft2Params &prm, in
 #pragma unroll
     for (int kq = 0; kq < H; ++kq) {
         const int kA = K + Q * kq;
-        gA[kq] = __ldg(gtab + kA);
-        gB[kq] = __ldg(gtab + ((n - kA) & (n - 1)));
+        gA[kq] = ldg_keep_f4(gtab + kA);
+        gB[kq] = ldg_keep_f4(gtab + ((n - kA) & (n - 1)));
     }
     auto rot_gain = [&](int kq, cx<f2> gA_, cx<f2> gB_, cx<f2> &rgA, cx<f2> &rgB) {
         if (prm.per_spectrum) {
