@@ -105,7 +105,11 @@ int fengine_process(fengine_t *fe, const void *in, void *out, int64_t n_spectra,
  * in pinned host memory and results go back to the host).
  * in_host / out_host  HOST pointers (pinned or pageable), same layouts as fengine_process.
  * Copies the input to device staging owned by the handle (grown on first use), runs the path on an
- * internal stream, copies the result back and synchronises before returning.
+ * internal stream, copies the result back and synchronises before returning.  On the tiled two-kernel path the
+ * call is cut into "host_chunks" pieces of spectra (option, default 8) and the upload of the rows a piece needs,
+ * its kernels and the download of its output records run on three streams, so that PCIe is busy in both
+ * directions under the kernels (the paper's chunked pipeline); pinned host buffers are needed
+ * for the copies to overlap.  The result is identical to fengine_process on the same data.
  */
 int fengine_process_host(fengine_t *fe, const void *in_host, void *out_host, int64_t n_spectra);
 
@@ -133,7 +137,7 @@ int fengine_debug_fir(fengine_t *fe, const void *in, float *g_out, int64_t n_spe
  * equal coarse delays), "fused" (0/1, default 0: run the pol-packed path as ONE persistent kernel whose FIR -> FFT
  * transposition goes through an L2-resident ring of scratch slots instead of a full-size HBM scratch; T = 4, 8, 16),
  * "ring_slots" / "lag" (ring depth D and FIR-to-FFT phase distance of the fused kernel, D >= lag + 2 is enforced),
- * "fused_ctas_per_sm" (0 = occupancy).  Returns INVALID_ARG for
+ * "fused_ctas_per_sm" (0 = occupancy), "host_chunks" (pieces of the fengine_process_host pipeline, 1 = no overlap).  Returns INVALID_ARG for
  * unknown keys. */
 int fengine_set_option(fengine_t *fe, const char *key, int64_t value);
 

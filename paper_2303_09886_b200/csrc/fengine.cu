@@ -31,6 +31,10 @@ struct fengine {
     bool tiled = false;             // tiled kernels cover this (n, T)
     bool packed_ok = false;         // pol-packed kernels (fe_fir2 / fe_fft2) cover this (n, T, P)
     bool pols_equal = true;         // both pols of every antenna have equal coarse delays (needed by them)
+    int32_t c_min = 0, c_max = 0;   // range of the coarse delays (host pipeline: which input rows a chunk needs)
+    int host_chunks = 8;            // option "host_chunks": pieces of the H2D / compute / D2H pipeline
+    cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
+    std::vector<cudaEvent_t> pipe_ev;
     bool allow_packed = true;       // option "pol_packed"
     int64_t n_coarse = 1, n_fine = 1;
     // device tables
@@ -369,10 +373,16 @@ int check_call(fengine *fe, const void *in, const void *out, int64_t S)
 }
 
 // the whole path; exactly one of out / out_f32 is non-null
-int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64_t S, cudaStream_t stream)
+// spectra [m_lo, m_hi) of a call of S spectra (m_hi < 0: all of them); a sub-range is only available on the tiled
+// two-kernel path (fengine_process_host pipelines over it)
+int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64_t S, cudaStream_t stream,
+                 int64_t m_lo = 0, int64_t m_hi = -1)
 {
-    fe->last_launches = 0;
-    if (S == 0) return FENGINE_OK;
+    if (m_hi < 0) m_hi = S;
+    if (m_lo == 0) fe->last_launches = 0;
+    if (S == 0 || m_hi <= m_lo) return FENGINE_OK;
+    if ((use_fused(fe) || !fe->tiled) && (m_lo != 0 || m_hi != S))
+        return fail(fe, FENGINE_ERR_STATE, "sub-range processing needs the tiled two-kernel path");
     const int streams = fe->A * fe->P;
 
     if (!fe->tiled) {
@@ -398,8 +408,9 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
         ++fe->last_launches;
     }
 
-    const int64_t chunk = fe->chunk_spectra > 0 ? std::min<int64_t>(fe->chunk_spectra, S) : S;
+    const int64_t chunk = fe->chunk_spectra > 0 ? std::min<int64_t>(fe->chunk_spectra, m_hi - m_lo) : m_hi - m_lo;
     const bool fused = use_fused(fe);
+
     int rc = fused ? FENGINE_OK : ensure_scratch(fe, (size_t)streams * chunk * fe->N);
     if (rc) return rc;
 
@@ -517,8 +528,8 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
         return FENGINE_OK;
     }
 
-    for (int64_t m0 = 0; m0 < S; m0 += chunk) {
-        const int64_t m1 = std::min(S, m0 + chunk);
+    for (int64_t m0 = m_lo; m0 < m_hi; m0 += chunk) {
+        const int64_t m1 = std::min(m_hi, m0 + chunk);
         fp.m_begin = xp.m_begin = fp2.m_begin = xp2.m_begin = m0;
         fp.m_end = xp.m_end = fp2.m_end = xp2.m_end = m1;
         cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
@@ -651,6 +662,9 @@ void fengine_destroy(fengine_t *fe)
     cudaFree(fe->d_stage_in);
     cudaFree(fe->d_stage_out);
     if (fe->host_stream) cudaStreamDestroy(fe->host_stream);
+    if (fe->s_h2d) cudaStreamDestroy(fe->s_h2d);
+    if (fe->s_d2h) cudaStreamDestroy(fe->s_d2h);
+    for (auto e : fe->pipe_ev) cudaEventDestroy(e);
     for (auto e : fe->ev_pool) cudaEventDestroy(e);
     for (auto e : fe->ev_used) cudaEventDestroy(e);
     cudaGetLastError();
@@ -675,6 +689,11 @@ int fengine_set_coarse_delays(fengine_t *fe, const int32_t *c, int64_t n_per_str
         fe->n_coarse = n_per_stream;
     }
     FE_CUDA(fe, cudaMemcpy(fe->d_coarse, c, sizeof(int32_t) * count, cudaMemcpyHostToDevice));
+    fe->c_min = fe->c_max = c[0];
+    for (size_t i = 1; i < count; ++i) {
+        fe->c_min = std::min(fe->c_min, c[i]);
+        fe->c_max = std::max(fe->c_max, c[i]);
+    }
     fe->pols_equal = true;                                  // the pol-packed kernels share one delay per antenna
     if (fe->P == 2)
         for (int a = 0; a < fe->A && fe->pols_equal; ++a)
@@ -765,9 +784,60 @@ int fengine_process_host(fengine_t *fe, const void *in_host, void *out_host, int
         }
         fe->stage_out_bytes = out_bytes;
     }
-    FE_CUDA(fe, cudaMemcpyAsync(fe->d_stage_in, in_host, in_bytes, cudaMemcpyHostToDevice, fe->host_stream));
     int rc = check_call(fe, fe->d_stage_in, fe->d_stage_out, n_spectra);
     if (rc) return rc;
+    // Pipeline (chunks are copied, processed and copied back concurrently): the call is cut into
+    // host_chunks pieces of spectra; the input rows a piece needs go up on one stream, the piece is processed on a
+    // second and its output records come down on a third, so that PCIe runs in both directions under the kernels.
+    const int K = fe->host_chunks;
+    if (fe->tiled && !use_fused(fe) && K > 1 && n_spectra >= 4 * (int64_t)K) {
+        const int64_t S = n_spectra, rows_in = S + fe->T - 1;
+        const size_t row_bytes = (size_t)fe->N / 4 * 5, stream_bytes = row_bytes * rows_in;
+        const int n_streams = fe->A * fe->P;
+        const size_t out_row = (size_t)fe->n * fe->P * 2, out_pitch = out_row * S;
+        if (!fe->s_h2d) FE_CUDA(fe, cudaStreamCreateWithFlags(&fe->s_h2d, cudaStreamNonBlocking));
+        if (!fe->s_d2h) FE_CUDA(fe, cudaStreamCreateWithFlags(&fe->s_d2h, cudaStreamNonBlocking));
+        while (fe->pipe_ev.size() < (size_t)(2 * K)) {
+            cudaEvent_t e;
+            FE_CUDA(fe, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            fe->pipe_ev.push_back(e);
+        }
+        // rows of the window of spectrum m: floor((N m - c) / N) .. floor((N m - c + N T - 1) / N)
+        const int64_t back = ((int64_t)fe->c_max + fe->N - 1) >> fe->lgN;               // ceil(c_max / N)
+        const int64_t fwd = (-(int64_t)fe->c_min + fe->N - 1) >> fe->lgN;               // ceil(-c_min / N)
+        (void)back;                                                                     // rows go up in order from 0
+        const int64_t per = (S + K - 1) / K;
+        int64_t copied = 0;
+        int64_t total_launches = 0;
+        const uint8_t *src = static_cast<const uint8_t *>(in_host);
+        int8_t *dst = static_cast<int8_t *>(out_host);
+        for (int k = 0; k * per < S; ++k) {
+            const int64_t m0 = k * per, m1 = std::min(S, m0 + per);
+            const int64_t need = std::min<int64_t>(rows_in, std::max<int64_t>(0, m1 + fe->T + fwd));
+            if (need > copied) {
+                FE_CUDA(fe, cudaMemcpy2DAsync(fe->d_stage_in + copied * row_bytes, stream_bytes, src + copied * row_bytes,
+                                              stream_bytes, (size_t)(need - copied) * row_bytes, n_streams,
+                                              cudaMemcpyHostToDevice, fe->s_h2d));
+                copied = need;
+            }
+            FE_CUDA(fe, cudaEventRecord(fe->pipe_ev[2 * k], fe->s_h2d));
+            FE_CUDA(fe, cudaStreamWaitEvent(fe->host_stream, fe->pipe_ev[2 * k], 0));
+            rc = process_impl(fe, fe->d_stage_in, fe->d_stage_out, nullptr, S, fe->host_stream, m0, m1);
+            if (rc) return rc;
+            total_launches += fe->last_launches;
+            fe->last_launches = 0;
+            FE_CUDA(fe, cudaEventRecord(fe->pipe_ev[2 * k + 1], fe->host_stream));
+            FE_CUDA(fe, cudaStreamWaitEvent(fe->s_d2h, fe->pipe_ev[2 * k + 1], 0));
+            FE_CUDA(fe, cudaMemcpy2DAsync(dst + m0 * out_row, out_pitch, fe->d_stage_out + m0 * out_row, out_pitch,
+                                          (size_t)(m1 - m0) * out_row, fe->A, cudaMemcpyDeviceToHost, fe->s_d2h));
+        }
+        fe->last_launches = total_launches;
+        FE_CUDA(fe, cudaStreamSynchronize(fe->s_h2d));
+        FE_CUDA(fe, cudaStreamSynchronize(fe->s_d2h));
+        FE_CUDA(fe, cudaStreamSynchronize(fe->host_stream));
+        return FENGINE_OK;
+    }
+    FE_CUDA(fe, cudaMemcpyAsync(fe->d_stage_in, in_host, in_bytes, cudaMemcpyHostToDevice, fe->host_stream));
     rc = process_impl(fe, fe->d_stage_in, fe->d_stage_out, nullptr, n_spectra, fe->host_stream);
     if (rc) return rc;
     FE_CUDA(fe, cudaMemcpyAsync(out_host, fe->d_stage_out, out_bytes, cudaMemcpyDeviceToHost, fe->host_stream));
@@ -869,6 +939,11 @@ int fengine_set_option(fengine_t *fe, const char *key, int64_t value)
     }
     if (!strcmp(key, "pol_packed")) {
         fe->allow_packed = value != 0;
+        return FENGINE_OK;
+    }
+    if (!strcmp(key, "host_chunks")) {
+        if (value < 1 || value > 1024) return fail(fe, FENGINE_ERR_INVALID_ARG, "host_chunks out of range");
+        fe->host_chunks = (int)value;
         return FENGINE_OK;
     }
     if (!strcmp(key, "fused")) {

@@ -294,6 +294,24 @@ def test_process_host_matches_device_path(torch, fb):
     np.testing.assert_array_equal(dev, pin_out.numpy())
 
 
+@pytest.mark.parametrize("n,A,S,crange,per_spectrum,chunks", [
+    (1024, 2, 150, (0, 2048), False, 8),
+    (4096, 2, 131, (-9000, 20000), False, 5),        # windows reach back and forward over several rows
+    (8192, 1, 70, (-20000, 3), True, 8),             # per-spectrum tables, non-packed kernels, reads ahead of the chunk
+    (1024, 1, 40, (0, 5), False, 64),                # more chunks asked for than 4 per spectrum allows: plain path
+])
+def test_process_host_pipeline_matches_device_path(torch, fb, n, A, S, crange, per_spectrum, chunks):
+    """fengine_process_host cuts the call into pieces and overlaps H2D, kernels and D2H."""
+    w = si.custom_workload(A=A, n=n, T=16, S=S, P=2, seed=41, per_spectrum=per_spectrum, coarse_range=crange)
+    fe = make_engine(fb, w, host_chunks=chunks)
+    dev = gpu_run(torch, fe, w, want=("int8",))["out"]
+    pin_in = torch.from_numpy(w.packed.reshape(-1)).pin_memory()
+    for _ in range(2):                               # staging buffers are reused by the second call
+        pin_out = torch.full(fe.output_shape(w.S), 77, dtype=torch.int8).pin_memory()
+        fe.process_host(pin_in, pin_out, w.S)
+        np.testing.assert_array_equal(dev, pin_out.numpy())
+
+
 def test_setters_take_effect_between_calls(torch, fb):
     w = si.make_workload(1, n_spectra=10)
     fe = make_engine(fb, w)
