@@ -340,9 +340,11 @@ __global__ void __launch_bounds__(Plan::tpf, FE_FFT2_MINB * ((512 / Plan::tpf) >
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int N = 2 * Plan::n;
-    const int a = blockIdx.y;
-    const int64_t m = prm.m_begin + blockIdx.x;
-    if (m >= prm.m_end) return;
+    // CTAs are issued in the reverse of the order in which the FIR kernel wrote the scratch (last antenna, last rows
+    // first): the most recently written ~100 MB are still in L2 when this kernel starts
+    const int a = (int)gridDim.y - 1 - (int)blockIdx.y;
+    const int64_t m = prm.m_end - 1 - (int64_t)blockIdx.x;
+    if (m < prm.m_begin) return;
     const float4 *grow = reinterpret_cast<const float4 *>(prm.g + ((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * (int64_t)N * 2);
     fft2_row<Plan, F32OUT>(prm, grow, smem_raw, a, m, threadIdx.x, [] {}, [] {});
 }
