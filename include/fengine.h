@@ -133,7 +133,7 @@ int fengine_debug_fir(fengine_t *fe, const void *in, float *g_out, int64_t n_spe
 /* Tuning knobs (optional; defaults are chosen at create).  key: "chunk_spectra" (spectra per
  * L2-resident chunk; 0 = whole call), "fir_rows" (spectra per FIR tile), "profile" (0/1, see below), "force_generic" (0/1: use the simple
  * one-thread-per-output kernels), "pol_packed" (0/1, default 1: allow the kernels that process both pols of an
- * antenna in packed FP32 lanes; they are used when n_pols = 2, n <= 4096 and the two pols of every antenna have
+ * antenna in packed FP32 lanes; they are used when n_pols = 2, n <= 8192 and the two pols of every antenna have
  * equal coarse delays), "fused" (0/1, default 0: run the pol-packed path as ONE persistent kernel whose FIR -> FFT
  * transposition goes through an L2-resident ring of scratch slots instead of a full-size HBM scratch; T = 4, 8, 16),
  * "ring_slots" / "lag" (ring depth D and FIR-to-FFT phase distance of the fused kernel, D >= lag + 2 is enforced),

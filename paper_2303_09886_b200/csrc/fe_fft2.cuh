@@ -26,21 +26,31 @@
 
 namespace fe {
 
-template <int N_CH, int R2_, int R3_, int TPF>
+// SW = 2 ("two sweeps", n = 8192): the first digit has radix 32; sweep h computes the top radix-2 stage of the
+// radix-32 butterfly on the fly while loading (a[j] = x[j] + x[j+16], or (x[j] - x[j+16]) W_32^j for h = 1) and then
+// runs the remaining n/2-point transform exactly like the one-sweep plan, producing the channels k = h (mod 2).
+// A channel and its mirror n - k have the same parity, so every sweep finishes its own channels.  The scratch row
+// is read once per sweep (the second read hits L2) and the exchange buffer stays at 64 KB: two CTAs per SM.
+template <int N_CH, int R2_, int R3_, int TPF, int SW_ = 1>
 struct Fft2Plan {
     static constexpr int n = N_CH;
+    static constexpr int SW = SW_;
+    static constexpr int nh = N_CH / SW_;                 // points of one sweep's transform
     static constexpr int R1 = 16, R2 = R2_, R3 = R3_;
     static constexpr int tpf = TPF;
-    static constexpr int M1 = N_CH / R1;                  // units per k1 block
+    static constexpr int M1 = nh / R1;                    // units per k1 block (= columns of pass 1)
     static constexpr int M2 = M1 / R2;                    // = R3
     static constexpr int Q = R1 * R2;                     // residues of the last pass
     static constexpr int blk = M1 + 1;                    // skewed block stride (units)
     static constexpr int units = R1 * blk;
-    static_assert(R1 * R2_ * R3_ == N_CH, "radices must multiply to n");
+    static_assert(SW_ == 1 || SW_ == 2, "one or two sweeps");
+    static_assert(R1 * R2_ * R3_ * SW_ == N_CH, "radices must multiply to n");
     static_assert(M2 == R3_, "three passes");
     static_assert(R3_ == 8 || R3_ == 16, "last radix 8 or 16");
     static_assert(TPF == Q && TPF % 32 == 0 && TPF >= 64, "one residue per thread in the last pass");
 };
+
+__device__ __forceinline__ cx<f2> unpack_unit_ld(float4 v) { return {f2(v.x, v.y), f2(v.z, v.w)}; }
 
 struct Fft2Params {
     const float *g;           // scratch rows a*chunk_cap + (m - m_begin), n units of 16 bytes
@@ -57,6 +67,45 @@ struct Fft2Params {
     int64_t m_begin, m_end, chunk_cap, n_spectra;
     int per_spectrum;
 };
+
+// top radix-2 stage of the radix-32 first digit, element J of sweep HS (compile-time J so that W_32^J is a constant)
+template <class Plan, int HS, int J>
+__device__ __forceinline__ void fft2_sweep_half(const float4 *__restrict__ grow, int col, cx<f2> (&a)[16])
+{
+    if constexpr (J < 16) {
+        const cx<f2> xu = unpack_unit_ld(ldg_stream_f4(grow + J * Plan::M1 + col));
+        const cx<f2> xv = unpack_unit_ld(ldg_stream_f4(grow + (J + 16) * Plan::M1 + col));
+        if constexpr (HS == 0)
+            a[J] = cadd(xu, xv);
+        else
+            a[J] = mul_w<32, J, f2>(csub(xu, xv));
+        fft2_sweep_half<Plan, HS, J + 1>(grow, col, a);
+    }
+}
+
+// pass 1 of sweep HS of a two-sweep plan: outputs k1 = 2 k'' + HS, twiddle W_n^{k1 col} as a running product
+template <class Plan, int HS>
+__device__ __forceinline__ void fft2_pass1_sweep(const float4 *__restrict__ grow, float4 *sm, const float2 *__restrict__ tw, int tid)
+{
+    constexpr int M1 = Plan::M1;
+    for (int col = tid; col < M1; col += Plan::tpf) {
+        cx<f2> a[16];
+        const float2 w1 = __ldg(tw + M1 + col);           // W_n^{col}
+        fft2_sweep_half<Plan, HS, 0>(grow, col, a);
+        Dif<16, f2>::run(a);
+        const float2 w2 = cmulf(w1, w1);
+        float2 wk = HS ? w1 : w2;
+#pragma unroll
+        for (int kk = 0; kk < 16; ++kk) {
+            cx<f2> y = a[kk];
+            if (2 * kk + HS > 0) {
+                y = cmul(a[kk], wk.x, wk.y);
+                if (kk + 1 < 16) wk = cmulf(wk, w2);
+            }
+            sm[kk * Plan::blk + col] = make_float4(y.re.v.x, y.re.v.y, y.im.v.x, y.im.v.y);
+        }
+    }
+}
 
 template <class Plan>
 __device__ __forceinline__ void fft2_pass1(const float4 *__restrict__ grow, float4 *sm, const float2 *__restrict__ tw, int tid)
@@ -100,7 +149,7 @@ template <class Plan>
 __device__ __forceinline__ void fft2_pass2(float4 *sm, const float2 *__restrict__ tw, int tid)
 {
     constexpr int R = Plan::R2, M2 = Plan::M2;
-    for (int b = tid; b < Plan::n / R; b += Plan::tpf) {
+    for (int b = tid; b < Plan::nh / R; b += Plan::tpf) {
         const int k1 = b / M2, lo = b - k1 * M2;
         float4 *col = sm + k1 * Plan::blk + lo;
         cx<f2> x[R];
@@ -175,22 +224,26 @@ __device__ __forceinline__ void fft2_epilogue(cx<f2> zk, cx<f2> zm, float2 tp, c
 // finishes the channels K + Q kq, kq < R3/2, together with their mirrors n - k, whose Z values are exactly the
 // upper half of residue Q - K.  Residue 0 mirrors onto itself with the index shifted by one (n - Q kq = Q (R3 - kq))
 // and also owns the self-mirrored channel n/2.
-template <class Plan, bool F32OUT>
+// Two-sweep plans (HS = sweep): residue K of sweep HS holds the channels k = HS + SW (K + Q kq); in the odd sweep
+// the mirror of residue K is residue Q - 1 - K and no residue mirrors onto itself.
+template <class Plan, bool F32OUT, int HS = 0>
 __device__ __forceinline__ void fft2_pass3(float4 *sm, const Fft2Params &prm, int a, int64_t m, int tid,
                                            const SpectrumPhase2 *sph)
 {
-    constexpr int R = Plan::R3, H = R / 2, Q = Plan::Q, n = Plan::n, N = 2 * n;
+    constexpr int R = Plan::R3, H = R / 2, Q = Plan::Q, n = Plan::n, N = 2 * n, SW = Plan::SW;
     static_assert(Plan::tpf == Q, "one residue per thread");
     const int K = tid;
+    const int k0 = HS + SW * K;                           // this thread's first channel
+    const bool special = HS == 0 && K == 0;
     float4 *mine = sm + (K & (Plan::R1 - 1)) * Plan::blk + (K / Plan::R1) * Plan::M2;
-    const int Kp = (Q - K) & (Q - 1);
+    const int Kp = HS ? Q - 1 - K : (Q - K) & (Q - 1);
     const float4 *theirs = sm + (Kp & (Plan::R1 - 1)) * Plan::blk + (Kp / Plan::R1) * Plan::M2;
 
     cx<f2> z[R];
 #pragma unroll
     for (int t = 0; t < R; ++t) z[t] = unpack_unit(mine[t]);
     Dif<R, f2>::run(z);
-    if (K == 0) {
+    if (special) {
 #pragma unroll
         for (int j = 0; j < H; ++j) mine[j] = pack_unit(z[(R - j) % R]);
         mine[H] = pack_unit(z[H]);
@@ -211,7 +264,7 @@ __device__ __forceinline__ void fft2_pass3(float4 *sm, const Fft2Params &prm, in
             const int cr = (int)(c & (N - 1));
             const double d = (double)prm.fine_d[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
             const double phi = (double)prm.fine_phi[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
-            const double t = -(d / (double)N) * (double)K - (double)((cr * K) & (N - 1)) / (double)N;
+            const double t = -(d / (double)N) * (double)k0 - (double)((cr * k0) & (N - 1)) / (double)N;
             double sp_, cp_;
             sincos(phi, &sp_, &cp_);
             e[p] = cmulf(phasor_turns(t), make_float2((float)cp_, (float)sp_));
@@ -220,9 +273,9 @@ __device__ __forceinline__ void fft2_pass3(float4 *sm, const Fft2Params &prm, in
     }
     // post-twiddle phasors without a table walk: (sin, cos)(2 pi (K + Q kq) / N) = the thread's own (sin, cos)(2 pi K / N)
     // rotated by the compile-time angle 2 pi kq Q / N (Q / N is 1/32 or 1/16), one table word per thread and spectrum
-    const float2 tpK = __ldg(prm.tpost + K);
+    const float2 tpK = __ldg(prm.tpost + k0);
     auto tp_of = [&](int kq) {
-        constexpr int st = 32 * Q / N;
+        constexpr int st = 32 * SW * Q / N;
         const float cphi = w32_cos(kq * st), sphi = w32_sin(kq * st);
         return make_float2(fmaf(tpK.x, cphi, tpK.y * sphi), fmaf(-tpK.x, sphi, tpK.y * cphi));
     };
@@ -234,7 +287,7 @@ __device__ __forceinline__ void fft2_pass3(float4 *sm, const Fft2Params &prm, in
     float4 gA[H], gB[H];
 #pragma unroll
     for (int kq = 0; kq < H; ++kq) {
-        const int kA = K + Q * kq;
+        const int kA = k0 + SW * Q * kq;
         gA[kq] = ldg_keep_f4(gtab + kA);
         gB[kq] = ldg_keep_f4(gtab + ((n - kA) & (n - 1)));
     }
@@ -257,13 +310,13 @@ __device__ __forceinline__ void fft2_pass3(float4 *sm, const Fft2Params &prm, in
     __syncthreads();                                      // upper halves are in the exchange buffer
 #pragma unroll
     for (int kq = 0; kq < H; ++kq) {
-        const int kA = K + Q * kq, kB = n - kA;            // kB == n for the DC channel (dropped Nyquist)
+        const int kA = k0 + SW * Q * kq, kB = n - kA;      // kB == n for the DC channel (dropped Nyquist)
         const cx<f2> zmk = unpack_unit(theirs[kq]);
         cx<f2> rgA, rgB;
         rot_gain(kq, unpack_unit(gA[kq]), unpack_unit(gB[kq]), rgA, rgB);
         fft2_epilogue<F32OUT>(z[kq], zmk, kq == 0 ? tpK : tp_of(kq), rgA, rgB, kA, kB, n, rec, yout);
     }
-    if (K == 0) {                                         // channel n/2 = Q * H mirrors onto itself
+    if (special) {                                        // channel n/2 = SW * Q * H mirrors onto itself
         const cx<f2> zh = unpack_unit(mine[H]);
         cx<f2> rgA, rgB;
         const cx<f2> gh = unpack_unit(__ldg(gtab + n / 2));
@@ -285,7 +338,7 @@ __device__ __forceinline__ void fft2_setup_phase(const Fft2Params &prm, Spectrum
         const double d = (double)prm.fine_d[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
         const double phi = (double)prm.fine_phi[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
         if (t < 16) {
-            const int k = Plan::Q * t;
+            const int k = Plan::SW * Plan::Q * t;
             const double tt = -(d / (double)N) * (double)k - (double)((cr * k) & (N - 1)) / (double)N;
             const float2 v = phasor_turns(tt);
             float *dst = reinterpret_cast<float *>(&sph->step[t]);
@@ -319,13 +372,29 @@ __device__ __forceinline__ void fft2_row(const Fft2Params &prm, const float4 *gr
     float4 *sm = reinterpret_cast<float4 *>(smem_raw);
     SpectrumPhase2 *sph = reinterpret_cast<SpectrumPhase2 *>(smem_raw + (size_t)Plan::units * 16);
     if (prm.per_spectrum) fft2_setup_phase<Plan>(prm, sph, a, m, tid);
-    fft2_pass1<Plan>(grow, sm, prm.tw1, tid);
-    __syncthreads();
-    after_load();
-    fft2_pass2<Plan>(sm, prm.tw2, tid);
-    __syncthreads();
-    after_pass2();
-    fft2_pass3<Plan, F32OUT>(sm, prm, a, m, tid, sph);
+    if constexpr (Plan::SW == 1) {
+        fft2_pass1<Plan>(grow, sm, prm.tw1, tid);
+        __syncthreads();
+        after_load();
+        fft2_pass2<Plan>(sm, prm.tw2, tid);
+        __syncthreads();
+        after_pass2();
+        fft2_pass3<Plan, F32OUT>(sm, prm, a, m, tid, sph);
+    } else {
+        fft2_pass1_sweep<Plan, 0>(grow, sm, prm.tw1, tid);
+        __syncthreads();
+        fft2_pass2<Plan>(sm, prm.tw2, tid);
+        __syncthreads();
+        fft2_pass3<Plan, F32OUT, 0>(sm, prm, a, m, tid, sph);
+        __syncthreads();                                  // the exchange buffer is reused by the odd sweep
+        fft2_pass1_sweep<Plan, 1>(grow, sm, prm.tw1, tid);
+        __syncthreads();
+        after_load();
+        fft2_pass2<Plan>(sm, prm.tw2, tid);
+        __syncthreads();
+        after_pass2();
+        fft2_pass3<Plan, F32OUT, 1>(sm, prm, a, m, tid, sph);
+    }
 }
 
 template <class Plan>

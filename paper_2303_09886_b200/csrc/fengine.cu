@@ -116,9 +116,10 @@ using Plan32768 = FftPlan<32768, 4, 32, 16, 8, 8, 512, 2>;     // two sweeps of 
 using Plan2_1024 = Fft2Plan<1024, 8, 8, 128>;
 using Plan2_2048 = Fft2Plan<2048, 8, 16, 128>;
 using Plan2_4096 = Fft2Plan<4096, 16, 16, 256>;
+using Plan2_8192 = Fft2Plan<8192, 16, 16, 256, 2>;    // two sweeps of 4096 points (fe_fft2.cuh)
 
 bool tiled_n(int n) { return n >= 1024 && n <= 32768; }
-bool packed_n(int n) { return n == 1024 || n == 2048 || n == 4096; }
+bool packed_n(int n) { return n == 1024 || n == 2048 || n == 4096 || n == 8192; }
 bool use_packed(const fengine *fe) { return fe->tiled && fe->packed_ok && fe->pols_equal && fe->allow_packed; }
 bool tiled_T(int T) { return T == 2 || T == 4 || T == 8 || T == 16; }
 
@@ -171,11 +172,15 @@ int launch_fft2_n(fengine *fe, const Fft2Params &prm, int64_t chunk_len, cudaStr
     case 1024: return launch_fft2<Plan2_1024, F32OUT>(fe, prm, chunk_len, stream);
     case 2048: return launch_fft2<Plan2_2048, F32OUT>(fe, prm, chunk_len, stream);
     case 4096: return launch_fft2<Plan2_4096, F32OUT>(fe, prm, chunk_len, stream);
+    case 8192: return launch_fft2<Plan2_8192, F32OUT>(fe, prm, chunk_len, stream);
     }
     return fail(fe, FENGINE_ERR_INVALID_ARG, "no pol-packed FFT plan for n=%d", fe->n);
 }
 
-bool use_fused(const fengine *fe) { return use_packed(fe) && fe->allow_fused && (fe->T == 4 || fe->T == 8 || fe->T == 16); }
+bool use_fused(const fengine *fe)
+{
+    return use_packed(fe) && fe->allow_fused && fe->n <= 4096 && (fe->T == 4 || fe->T == 8 || fe->T == 16);
+}
 
 template <int T, class Plan, bool F32OUT>
 int launch_fused(fengine *fe, const FusedParams &prm, cudaStream_t stream)
@@ -635,6 +640,7 @@ fengine_t *fengine_create_batched(int n_antennas, int n_channels, int taps, int 
             case 1024: rc = build_tables2<Plan2_1024>(fe); break;
             case 2048: rc = build_tables2<Plan2_2048>(fe); break;
             case 4096: rc = build_tables2<Plan2_4096>(fe); break;
+            case 8192: rc = build_tables2<Plan2_8192>(fe); break;
             }
         }
         ok = rc == FENGINE_OK;
