@@ -485,9 +485,10 @@ __global__ void __launch_bounds__(Plan::tpf, (512 / Plan::tpf) > 0 ? (512 / Plan
     SpectrumPhase *sph = reinterpret_cast<SpectrumPhase *>(smem_raw + (size_t)Plan::units * 16 + (size_t)(n / SW) * P * 2);
 
     const int tid = threadIdx.x;
-    const int a = blockIdx.y;
-    const int64_t m = prm.m_begin + blockIdx.x;
-    if (m >= prm.m_end) return;
+    // reverse of the FIR kernel's write order: the newest scratch rows are still in L2 (see fft2_kernel)
+    const int a = (int)gridDim.y - 1 - (int)blockIdx.y;
+    const int64_t m = prm.m_end - 1 - (int64_t)blockIdx.x;
+    if (m < prm.m_begin) return;
 
     for (int sweep = 0; sweep < SW; ++sweep) {
         for (int pol = 0; pol < P; ++pol) {
