@@ -113,6 +113,18 @@ int fengine_process(fengine_t *fe, const void *in, void *out, int64_t n_spectra,
  */
 int fengine_process_host(fengine_t *fe, const void *in_host, void *out_host, int64_t n_spectra);
 
+/*
+ * fengine_process_heaps -- the same path with the output in the channel-major heaps the X-engines consume
+ * ("each heap contains data for 256 spectra ... a c x 256 x 2 array of Gaussian integers";
+ * the post-processing transposes from time-major to channel-major within each heap).
+ * in         DEVICE, as fengine_process.
+ * heaps_out  DEVICE, 16-byte aligned, [A][ceil(S / 256)][n][256][P][2] int8: heap h of antenna a holds spectra
+ *            256 h .. 256 h + 255, channel-major; spectra past S in the last heap are written as zero.
+ * The time-major records are produced by the kernels of fengine_process into a buffer owned by the handle (sized
+ * at the first call) and transposed through shared memory by one more kernel; n >= 32.
+ */
+int fengine_process_heaps(fengine_t *fe, const void *in, void *heaps_out, int64_t n_spectra, void *stream);
+
 /* Human-readable description of the last error on this handle ("" if none). */
 const char *fengine_last_error(const fengine_t *fe);
 

@@ -15,7 +15,7 @@ EXPORTED_SYMBOLS = [
     "fengine_create", "fengine_create_batched", "fengine_destroy", "fengine_set_coarse_delays",
     "fengine_set_fine_delays", "fengine_set_gains", "fengine_process", "fengine_process_host",
     "fengine_last_error", "fengine_process_f32", "fengine_debug_unpack", "fengine_debug_fir",
-    "fengine_set_option", "fengine_last_launch_count", "fengine_profile_read",
+    "fengine_set_option", "fengine_last_launch_count", "fengine_profile_read", "fengine_process_heaps",
 ]
 
 STATUS = {0: "OK", 1: "INVALID_ARG", 2: "ALLOC", 3: "CUDA", 4: "STATE"}
@@ -52,6 +52,7 @@ def lib() -> C.CDLL:
         L.fengine_set_gains.argtypes = [vp, vp]
         L.fengine_process.argtypes = [vp, vp, vp, i64, vp]
         L.fengine_process_host.argtypes = [vp, vp, vp, i64]
+        L.fengine_process_heaps.argtypes = [vp, vp, vp, i64, vp]
         L.fengine_process_f32.argtypes = [vp, vp, vp, i64, vp]
         L.fengine_debug_unpack.argtypes = [vp, vp, vp, i64, vp]
         L.fengine_debug_fir.argtypes = [vp, vp, vp, i64, vp]
@@ -147,6 +148,14 @@ class FEngine:
     def process(self, inp, out, n_spectra: int, stream=None):
         """fengine_process: device tensors (uint8 in, int8 out); asynchronous on `stream`."""
         self._check(self._lib.fengine_process(self._h, _dev_ptr(inp), _dev_ptr(out), n_spectra, _stream_handle(stream)))
+
+    def heaps_shape(self, n_spectra: int):
+        return (self.A, (n_spectra + 255) // 256, self.n, 256, self.P, 2)
+
+    def process_heaps(self, inp, heaps_out, n_spectra: int, stream=None):
+        """fengine_process_heaps: channel-major heaps of 256 spectra (int8, shape heaps_shape(n_spectra))."""
+        self._check(self._lib.fengine_process_heaps(self._h, _dev_ptr(inp), _dev_ptr(heaps_out), n_spectra,
+                                                    _stream_handle(stream)))
 
     def process_f32(self, inp, out_f32, n_spectra: int, stream=None):
         self._check(self._lib.fengine_process_f32(self._h, _dev_ptr(inp), _dev_ptr(out_f32), n_spectra,

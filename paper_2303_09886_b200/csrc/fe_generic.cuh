@@ -129,4 +129,26 @@ __global__ void unrotate_kernel(const float *gp, float *g_out, const int32_t *co
     }
 }
 
+// Channel-major output heaps: the X-engines consume, per antenna and per group of 256 spectra,
+// a [channel][256 spectra][pol] array of Gaussian integers.  rec is the time-major output [A][S][n] of words
+// (one word = the P (re, im) byte pairs of a channel), heaps is [A][ceil(S/256)][n][256] words; spectra past S in
+// the last heap are zero.  32 x 32-word tiles through shared memory, both sides coalesced.
+template <typename Word>
+__global__ void heaps_transpose_kernel(const Word *__restrict__ rec, Word *__restrict__ heaps, int64_t S, int n)
+{
+    __shared__ Word tile[32][33];
+    const int64_t n_heaps = (S + 255) / 256;
+    const int a = blockIdx.z / (int)n_heaps, h = blockIdx.z - a * (int)n_heaps;
+    const int k0 = blockIdx.x * 32, s0 = blockIdx.y * 32;             // channel / in-heap spectrum of the tile
+    const Word *src = rec + ((int64_t)a * S + (int64_t)h * 256) * n;
+    Word *dst = heaps + ((int64_t)a * n_heaps + h) * (int64_t)n * 256;
+    for (int j = threadIdx.y; j < 32; j += blockDim.y) {
+        const int64_t m = (int64_t)h * 256 + s0 + j;
+        tile[j][threadIdx.x] = m < S ? src[(int64_t)(s0 + j) * n + k0 + threadIdx.x] : Word(0);
+    }
+    __syncthreads();
+    for (int j = threadIdx.y; j < 32; j += blockDim.y)
+        dst[(int64_t)(k0 + j) * 256 + s0 + threadIdx.x] = tile[threadIdx.x][j];
+}
+
 }  // namespace fe

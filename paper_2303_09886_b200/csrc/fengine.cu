@@ -65,6 +65,8 @@ struct fengine {
     uint8_t *d_stage_in = nullptr;
     int8_t *d_stage_out = nullptr;
     size_t stage_in_bytes = 0, stage_out_bytes = 0;
+    int8_t *d_rec = nullptr;        // time-major records of fengine_process_heaps
+    size_t rec_bytes = 0;
     cudaStream_t host_stream = nullptr;
     // options
     int64_t chunk_spectra = 0;      // 0 = whole call in one chunk
@@ -677,6 +679,7 @@ void fengine_destroy(fengine_t *fe)
     cudaFree(fe->d_scratch);
     cudaFree(fe->d_ring);
     cudaFree(fe->d_ctl);
+    cudaFree(fe->d_rec);
     cudaFree(fe->d_stage_in);
     cudaFree(fe->d_stage_out);
     if (fe->host_stream) cudaStreamDestroy(fe->host_stream);
@@ -770,6 +773,41 @@ int fengine_process(fengine_t *fe, const void *in, void *out, int64_t n_spectra,
     int rc = check_call(fe, in, out, n_spectra);
     if (rc) return rc;
     return process_impl(fe, in, static_cast<int8_t *>(out), nullptr, n_spectra, static_cast<cudaStream_t>(stream));
+}
+
+int fengine_process_heaps(fengine_t *fe, const void *in, void *heaps_out, int64_t n_spectra, void *stream)
+{
+    int rc = check_call(fe, in, heaps_out, n_spectra);
+    if (rc || n_spectra == 0) return rc;
+    if (fe->n < 32) return fail(fe, FENGINE_ERR_INVALID_ARG, "heaps need n >= 32");
+    const size_t bytes = (size_t)fe->A * n_spectra * fe->n * fe->P * 2;
+    if (bytes > fe->rec_bytes) {
+        if (fe->d_rec) {
+            FE_CUDA(fe, cudaDeviceSynchronize());
+            cudaFree(fe->d_rec);
+            fe->d_rec = nullptr;
+            fe->rec_bytes = 0;
+        }
+        if (cudaMalloc(&fe->d_rec, bytes) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(fe, FENGINE_ERR_ALLOC, "cannot allocate %zu bytes for the time-major records", bytes);
+        }
+        fe->rec_bytes = bytes;
+    }
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    rc = process_impl(fe, in, fe->d_rec, nullptr, n_spectra, s);
+    if (rc) return rc;
+    const int64_t n_heaps = (n_spectra + 255) / 256;
+    dim3 grid((unsigned)(fe->n / 32), 8, (unsigned)(fe->A * n_heaps)), block(32, 8);
+    if (fe->P == 2)
+        heaps_transpose_kernel<uint32_t><<<grid, block, 0, s>>>(reinterpret_cast<const uint32_t *>(fe->d_rec),
+                                                                static_cast<uint32_t *>(heaps_out), n_spectra, fe->n);
+    else
+        heaps_transpose_kernel<uint16_t><<<grid, block, 0, s>>>(reinterpret_cast<const uint16_t *>(fe->d_rec),
+                                                                static_cast<uint16_t *>(heaps_out), n_spectra, fe->n);
+    ++fe->last_launches;
+    FE_CUDA(fe, cudaGetLastError());
+    return FENGINE_OK;
 }
 
 int fengine_process_host(fengine_t *fe, const void *in_host, void *out_host, int64_t n_spectra)

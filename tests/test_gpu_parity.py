@@ -312,6 +312,27 @@ def test_process_host_pipeline_matches_device_path(torch, fb, n, A, S, crange, p
         np.testing.assert_array_equal(dev, pin_out.numpy())
 
 
+@pytest.mark.parametrize("n,A,P,S", [(1024, 2, 2, 300), (4096, 1, 2, 256), (1024, 1, 1, 70), (64, 2, 2, 513)])
+def test_channel_major_heaps_are_the_transposed_records(torch, fb, n, A, P, S):
+    """fengine_process_heaps: [A][heap][channel][256 spectra][pol][re,im], zero past S."""
+    w = si.custom_workload(A=A, n=n, T=4 if n == 64 else 16, S=S, P=P, seed=43, random_weights=(n <= 64))
+    fe = make_engine(fb, w)
+    ref = oracle_run(w)["out"]                                   # [A][S][n][P][2], from the oracle
+    n_heaps = (S + 255) // 256
+    want = np.zeros((A, n_heaps * 256, n, P, 2), np.int8)
+    want[:, :S] = ref
+    want = want.reshape(A, n_heaps, 256, n, P, 2).transpose(0, 1, 3, 2, 4, 5)
+    d_in = torch.from_numpy(w.packed.reshape(-1)).cuda()
+    d_heaps = torch.full(fe.heaps_shape(S), 99, dtype=torch.int8, device="cuda")
+    fe.process_heaps(d_in, d_heaps, S)
+    torch.cuda.synchronize()
+    got = d_heaps.cpu().numpy()
+    assert got.shape == want.shape
+    diff = np.abs(got.astype(np.int32) - want.astype(np.int32))
+    assert diff.max() <= 1 and np.count_nonzero(diff) <= max(1, int(1e-4 * diff.size))
+    assert not got[:, -1, :, S - 256 * (n_heaps - 1):].any() or S % 256 == 0     # tail of the last heap is zero
+
+
 def test_setters_take_effect_between_calls(torch, fb):
     w = si.make_workload(1, n_spectra=10)
     fe = make_engine(fb, w)
