@@ -12,10 +12,6 @@
 #error "fengine kernels are written for sm_100a (B200) only"
 #endif
 
-#ifndef FE_GAIN_EVICT_LAST
-#define FE_GAIN_EVICT_LAST 1
-#endif
-
 namespace fe {
 
 struct f2 {
@@ -80,12 +76,8 @@ __device__ __forceinline__ float4 ldg_stream_f4(const float4 *p)
 __device__ __forceinline__ float4 ldg_keep_f4(const float4 *p)
 {
     float4 v;
-#if FE_GAIN_EVICT_LAST
     asm volatile("ld.global.nc.L1::evict_last.v4.f32 {%0,%1,%2,%3}, [%4];"
                  : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
-#else
-    v = __ldg(p);
-#endif
     return v;
 }
 __device__ __forceinline__ void stg_stream_f4(float4 *p, float4 v)

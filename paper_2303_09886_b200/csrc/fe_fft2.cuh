@@ -17,12 +17,6 @@
 #include "fe_common.cuh"
 #include "fe_fft.cuh"
 
-#ifndef FE_FFT2_MINB
-#define FE_FFT2_MINB 2
-#endif
-#ifndef FE_TW1_POWERS
-#define FE_TW1_POWERS 1
-#endif
 
 namespace fe {
 
@@ -120,7 +114,6 @@ __device__ __forceinline__ void fft2_pass1(const float4 *__restrict__ grow, floa
             x[t].im = f2(v.z, v.w);
         }
         Dif<R, f2>::run(x);
-#if FE_TW1_POWERS
         // W_n^{k col}, k = 1..15, as powers of the one table word W_n^{col} (product tree of depth <= 4: the
         // rounding error stays below 5e-7, far inside the 1e-4 budget), so pass 1 reads 8 bytes of table per
         // butterfly instead of 120 and the table never competes with the gain table for the L1
@@ -128,17 +121,11 @@ __device__ __forceinline__ void fft2_pass1(const float4 *__restrict__ grow, floa
         w[1] = __ldg(tw + M1 + col);
 #pragma unroll
         for (int k = 2; k < R; ++k) w[k] = cmulf(w[k / 2], w[k - k / 2]);
-#endif
 #pragma unroll
         for (int k = 0; k < R; ++k) {
             cx<f2> y = x[k];
             if (k > 0) {
-#if FE_TW1_POWERS
                 y = cmul(x[k], w[k].x, w[k].y);
-#else
-                const float2 wk = __ldg(tw + k * M1 + col);
-                y = cmul(x[k], wk.x, wk.y);
-#endif
             }
             sm[k * Plan::blk + col] = make_float4(y.re.v.x, y.re.v.y, y.im.v.x, y.im.v.y);
         }
@@ -405,7 +392,7 @@ constexpr size_t fft2_smem_bytes()
 
 // One CTA per (antenna, spectrum), both pols.
 template <class Plan, bool F32OUT>
-__global__ void __launch_bounds__(Plan::tpf, FE_FFT2_MINB * ((512 / Plan::tpf) > 0 ? (512 / Plan::tpf) : 1) / 2) fft2_kernel(const Fft2Params prm)
+__global__ void __launch_bounds__(Plan::tpf, (512 / Plan::tpf) > 0 ? (512 / Plan::tpf) : 1) fft2_kernel(const Fft2Params prm)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int N = 2 * Plan::n;

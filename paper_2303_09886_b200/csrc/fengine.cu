@@ -158,8 +158,6 @@ int launch_fft2(fengine *fe, const Fft2Params &prm, int64_t chunk_len, cudaStrea
     static bool attr_set = false;
     if (!attr_set) {
         FE_CUDA(fe, cudaFuncSetAttribute(fft2_kernel<Plan, F32OUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        if (const char *cv = getenv("FE_FFT2_CARVEOUT"))
-            FE_CUDA(fe, cudaFuncSetAttribute(fft2_kernel<Plan, F32OUT>, cudaFuncAttributePreferredSharedMemoryCarveout, atoi(cv)));
         attr_set = true;
     }
     dim3 grid((unsigned)chunk_len, (unsigned)fe->A);
@@ -192,7 +190,6 @@ int launch_fused(fengine *fe, const FusedParams &prm, cudaStream_t stream)
     if (!ctas_per_sm) {
         FE_CUDA(fe, cudaFuncSetAttribute(fused2_kernel<T, Plan, F32OUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         FE_CUDA(fe, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, fused2_kernel<T, Plan, F32OUT>, Plan::tpf, smem));
-        if (getenv("FE_DEBUG")) fprintf(stderr, "fused2_kernel: occupancy %d CTAs/SM, smem %zu\n", ctas_per_sm, smem);
         if (ctas_per_sm < 1) ctas_per_sm = 1;
     }
     const int per_sm = fe->fused_ctas_per_sm > 0 ? fe->fused_ctas_per_sm : ctas_per_sm;
