@@ -145,6 +145,7 @@ def main():
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--n-channels", type=int, default=None, help="sweep point for config 5")
     ap.add_argument("--n-spectra", type=int, default=None, help="shrink the batch (debugging only)")
+    ap.add_argument("--taps", type=int, default=None, help="override T (tap sweep of PAPER.md:235-249; 2, 4, 8, 16, 32)")
     ap.add_argument("--chunk-spectra", type=int, default=None)
     ap.add_argument("--fir-rows", type=int, default=None)
     ap.add_argument("--opt", action="append", default=[], help="library option key=value (fengine_set_option), repeatable")
@@ -171,7 +172,7 @@ def main():
     fb.lib()                                             # fail loudly if the CUDA library is missing
     # Streams are independent: every rank runs the full configuration on its own antennas
     # (weak scaling, no data-path collective).  Different seed per rank = different antennas.
-    w = si.make_workload(args.config, n_spectra=args.n_spectra, n_channels=args.n_channels, seed=rank)
+    w = si.make_workload(args.config, n_spectra=args.n_spectra, n_channels=args.n_channels, seed=rank, taps=args.taps)
     fe = fb.FEngine(w.n, w.T, w.P, w.weights, n_antennas=w.A)
     fe.set_coarse_delays(w.coarse)
     fe.set_fine_delays(w.fine_delay, w.phase)

@@ -46,7 +46,9 @@ enum {
  * polarisations of one antenna).  Same as fengine_create_batched(1, ...).
  *
  * n_channels  n, a power of two, 8 <= n <= 32768 (1024, 4096, 8192, 32768).
- * taps        T, 1 <= T <= 32 (PAPER.md:39: up to 16; :245 measures 32).
+ * taps        T, 1 <= T <= 32 (PAPER.md:39: up to 16; :245 measures 32).  T = 2, 4, 8, 16 run the tiled kernels for
+ *             n >= 1024; T = 32 runs them on the pol-packed path (n_pols = 2, n <= 8192, equal coarse delays in
+ *             both pols); every other shape runs the generic one-thread-per-output kernels (slow, for tests).
  * n_pols      1 or 2.
  * weights     HOST, N*T floats, N = 2n, flat time order weights[t + N*j] = w[t][j] of Eq. (1)
  *             (BASELINE.json configs[0]).  Must be finite.  Copied.

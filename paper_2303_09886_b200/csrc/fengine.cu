@@ -21,6 +21,7 @@
 #include "fe_fft2.cuh"
 #include "fe_fir.cuh"
 #include "fe_fir2.cuh"
+#include "fe_fir3.cuh"
 #include "fe_fused.cuh"
 #include "fe_generic.cuh"
 
@@ -123,7 +124,7 @@ using Plan2_8192 = Fft2Plan<8192, 16, 16, 256, 2>;    // two sweeps of 4096 poin
 bool tiled_n(int n) { return n >= 1024 && n <= 32768; }
 bool packed_n(int n) { return n == 1024 || n == 2048 || n == 4096 || n == 8192; }
 bool use_packed(const fengine *fe) { return fe->tiled && fe->packed_ok && fe->pols_equal && fe->allow_packed; }
-bool tiled_T(int T) { return T == 2 || T == 4 || T == 8 || T == 16; }
+bool tiled_T(int T) { return T == 2 || T == 4 || T == 8 || T == 16 || T == 32; }
 
 template <class Plan>
 int build_tables(fengine *fe)
@@ -177,6 +178,8 @@ int launch_fft2_n(fengine *fe, const Fft2Params &prm, int64_t chunk_len, cudaStr
     return fail(fe, FENGINE_ERR_INVALID_ARG, "no pol-packed FFT plan for n=%d", fe->n);
 }
 
+// T = 32 exists only as the one-column pol-packed FIR (fe_fir3.cuh); other 32-tap engines run the generic kernels
+bool use_tiled(const fengine *fe) { return fe->tiled && (fe->T != 32 || use_packed(fe)); }
 bool use_fused(const fengine *fe)
 {
     return use_packed(fe) && fe->allow_fused && fe->n <= 4096 && (fe->T == 4 || fe->T == 8 || fe->T == 16);
@@ -261,6 +264,12 @@ int ensure_fused(fengine *fe, int64_t S, int C, int D)
 
 int launch_fir2(fengine *fe, const Fir2Params &prm, int64_t chunk_len, cudaStream_t stream)
 {
+    if (fe->T == 32) {                                      // one column per thread: 32 taps stay in registers
+        dim3 grid3((unsigned)(fe->N / kFir3Threads), (unsigned)((chunk_len + prm.rows_per_tile - 1) / prm.rows_per_tile),
+                   (unsigned)fe->A);
+        fir3_kernel<32><<<grid3, kFir3Threads, 0, stream>>>(prm);
+        return FENGINE_OK;
+    }
     dim3 grid((unsigned)(fe->n / kFir2Threads), (unsigned)((chunk_len + prm.rows_per_tile - 1) / prm.rows_per_tile),
               (unsigned)fe->A);
     switch (fe->T) {
@@ -397,11 +406,11 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
     if (m_hi < 0) m_hi = S;
     if (m_lo == 0) fe->last_launches = 0;
     if (S == 0 || m_hi <= m_lo) return FENGINE_OK;
-    if ((use_fused(fe) || !fe->tiled) && (m_lo != 0 || m_hi != S))
+    if ((use_fused(fe) || !use_tiled(fe)) && (m_lo != 0 || m_hi != S))
         return fail(fe, FENGINE_ERR_STATE, "sub-range processing needs the tiled two-kernel path");
     const int streams = fe->A * fe->P;
 
-    if (!fe->tiled) {
+    if (!use_tiled(fe)) {
         int rc = ensure_scratch(fe, (size_t)streams * S * fe->N);
         if (rc) return rc;
         const GenParams gp = gen_params(fe, in, S);
@@ -843,7 +852,7 @@ int fengine_process_host(fengine_t *fe, const void *in_host, void *out_host, int
     // host_chunks pieces of spectra; the input rows a piece needs go up on one stream, the piece is processed on a
     // second and its output records come down on a third, so that PCIe runs in both directions under the kernels.
     const int K = fe->host_chunks;
-    if (fe->tiled && !use_fused(fe) && K > 1 && n_spectra >= 4 * (int64_t)K) {
+    if (use_tiled(fe) && !use_fused(fe) && K > 1 && n_spectra >= 4 * (int64_t)K) {
         const int64_t S = n_spectra, rows_in = S + fe->T - 1;
         const size_t row_bytes = (size_t)fe->N / 4 * 5, stream_bytes = row_bytes * rows_in;
         const int n_streams = fe->A * fe->P;
@@ -922,7 +931,7 @@ int fengine_debug_fir(fengine_t *fe, const void *in, float *g_out, int64_t n_spe
     if (rc || n_spectra == 0) return rc;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const int64_t total = (int64_t)fe->A * fe->P * n_spectra * fe->N;
-    if (!fe->tiled) {
+    if (!use_tiled(fe)) {
         gen_fir_kernel<<<gen_grid(total), 256, 0, s>>>(gen_params(fe, in, n_spectra), g_out);
     } else if (use_packed(fe)) {
         rc = ensure_scratch(fe, (size_t)total);

@@ -127,17 +127,17 @@ def _random_gains(prng, A, P, n):
 
 def make_workload(config: int, n_spectra: int | None = None, n_antennas: int | None = None,
                   n_channels: int | None = None, seed: int = 0, keep_samples: bool = False,
-                  sigma: float | None = None) -> Workload:
+                  sigma: float | None = None, taps: int | None = None) -> Workload:
     """Build the synthetic stand-in for BASELINE.json config `config` (1..5).
 
     n_spectra / n_antennas shrink the batch (same distributions) so that the oracle finishes in
     seconds; n_channels selects the sweep point of config 5.  `sigma` overrides the noise level
-    (config 4 variant 4b uses sigma=182, R17).
+    (config 4 variant 4b uses sigma=182, R17).  `taps` overrides T (the paper's tap sweep).
     """
     shp = dict(CONFIG_SHAPES[config])
     A = n_antennas or shp["A"]
     n = n_channels or shp["n"]
-    T = shp["T"]
+    T = taps or shp["T"]
     P = 2
     N = 2 * n
     if n_spectra is None:

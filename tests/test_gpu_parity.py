@@ -120,7 +120,7 @@ def test_unpack_and_coarse_delay_bit_exact(torch, fb, case):
 
 
 @pytest.mark.parametrize("n,T,c", [(1024, 16, 0), (1024, 16, 3), (4096, 16, 4093), (4096, 8, -5), (2048, 4, 70001),
-                                    (8192, 16, 16382), (1024, 2, 2047)])
+                                    (8192, 16, 16382), (1024, 2, 2047), (4096, 32, 777), (1024, 32, -3000)])
 def test_tiled_fir_unpack_is_bit_exact_with_one_hot_weights(torch, fb, n, T, c):
     """weights = 1 at one tap: the tiled FIR must return the delayed integer samples exactly."""
     N = 2 * n
@@ -147,7 +147,7 @@ def test_tiled_fir_unpack_is_bit_exact_with_one_hot_weights(torch, fb, n, T, c):
 # ----------------------------------------------------------------------------------------------
 # FIR (Eq. 1) against the oracle's direct sum
 # ----------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("n,T,per_spectrum", [(1024, 16, False), (4096, 16, True), (64, 5, False)])
+@pytest.mark.parametrize("n,T,per_spectrum", [(1024, 16, False), (4096, 16, True), (64, 5, False), (2048, 32, True)])
 def test_fir_matches_oracle(torch, fb, n, T, per_spectrum):
     w = si.custom_workload(A=2, n=n, T=T, S=37, seed=24, per_spectrum=per_spectrum, random_weights=True,
                            coarse_range=(-7, 2 * n + 50))
@@ -226,6 +226,23 @@ def test_shapes_and_edges(torch, fb, n, T, S, A, P, per_spectrum, crange):
     got = gpu_run(torch, fe, w)
     ref = oracle_run(w)
     check_parity(got, ref, f"n={n} T={T} S={S} A={A} P={P}")
+
+
+@pytest.mark.parametrize("n,S,A,per_spectrum,equal_pols", [
+    (1024, 70, 2, False, True),
+    (4096, 140, 1, True, True),                      # per-spectrum delays: runs restart inside a tile
+    (8192, 40, 1, False, True),
+    (32, 9, 1, False, False),                        # unequal pols: 32 taps fall back to the generic kernels
+])
+def test_32_taps(torch, fb, n, S, A, per_spectrum, equal_pols):
+    """T = 32 runs the one-column pol-packed FIR (fe_fir3.cuh)."""
+    w = si.custom_workload(A=A, n=n, T=32, S=S, P=2, seed=47, per_spectrum=per_spectrum, coarse_range=(-n, 4 * n),
+                           random_weights=(n <= 64))
+    if equal_pols:
+        w.coarse[:, 1] = w.coarse[:, 0]
+    fe = make_engine(fb, w)
+    got = gpu_run(torch, fe, w)
+    check_parity(got, oracle_run(w), f"T=32 n={n}")
 
 
 def test_generic_and_tiled_kernels_agree(torch, fb):
