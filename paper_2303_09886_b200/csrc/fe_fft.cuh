@@ -133,11 +133,16 @@ struct FftPlan {
 
 // unit address swizzle: XOR the low 3 bits with the low 3 bits of digit 1 (conflict-free 128-bit
 // accesses both for "8 consecutive pair indices" (passes 1..q-1) and "8 consecutive k1" (last pass))
+// Plans whose third pass has a stride of 4 units (n = 16384, 32768) would see units 32 apart (the same banks) in one
+// quarter-warp of that pass; XORing bit 5 into bit 2 removes that 2-way conflict at the price of a 1.1-way one on the
+// last pass's loads (checked for every plan and pass with a host-side model of the bank mapping).
 template <class Plan>
 __device__ __forceinline__ int swz(int lin)
 {
     const int d1 = lin / Plan::S(1);
-    return lin ^ (d1 & 7);
+    int s = lin ^ (d1 & 7);
+    if constexpr (Plan::q == 4 && Plan::S(3) == 4) s ^= ((lin >> 5) & 1) << 2;
+    return s;
 }
 
 struct FftTables {
