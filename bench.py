@@ -145,6 +145,7 @@ def main():
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--n-channels", type=int, default=None, help="sweep point for config 5")
     ap.add_argument("--n-spectra", type=int, default=None, help="shrink the batch (debugging only)")
+    ap.add_argument("--sample-bits", type=int, default=10, help="input sample width (bit-depth sweep of PAPER.md:273-279)")
     ap.add_argument("--taps", type=int, default=None, help="override T (tap sweep of PAPER.md:235-249; 2, 4, 8, 16, 32)")
     ap.add_argument("--chunk-spectra", type=int, default=None)
     ap.add_argument("--fir-rows", type=int, default=None)
@@ -172,11 +173,13 @@ def main():
     fb.lib()                                             # fail loudly if the CUDA library is missing
     # Streams are independent: every rank runs the full configuration on its own antennas
     # (weak scaling, no data-path collective).  Different seed per rank = different antennas.
-    w = si.make_workload(args.config, n_spectra=args.n_spectra, n_channels=args.n_channels, seed=rank, taps=args.taps)
+    w = si.make_workload(args.config, n_spectra=args.n_spectra, n_channels=args.n_channels, seed=rank, taps=args.taps, bits=args.sample_bits)
     fe = fb.FEngine(w.n, w.T, w.P, w.weights, n_antennas=w.A)
     fe.set_coarse_delays(w.coarse)
     fe.set_fine_delays(w.fine_delay, w.phase)
     fe.set_gains(w.gains)
+    if args.sample_bits != 10:
+        fe.set_option("sample_bits", args.sample_bits)
     if args.chunk_spectra is not None:
         fe.set_option("chunk_spectra", args.chunk_spectra)
     if args.fir_rows is not None:
@@ -242,9 +245,10 @@ def main():
     fir_avg, fft_avg = fir_ms / max(n_fir, 1), fft_ms / max(n_fft, 1)
     launches_per_step = max(n_fir // max(args.steps, 1), 1)
     dom_name, dom_avg = ("fft_kernel", fft_avg) if fft_avg >= fir_avg else ("fir_kernel", fir_avg)
-    alg_bytes_launch = ALG_BYTES_PER_DUALPOL_SAMPLE * units_per_step / launches_per_step
+    alg_bytes_per_unit = 2.0 * (args.sample_bits / 8.0 + 1.0)      # 4.5 at 10 bits (ALG_BYTES_PER_DUALPOL_SAMPLE)
+    alg_bytes_launch = alg_bytes_per_unit * units_per_step / launches_per_step
     achieved = alg_bytes_launch / (dom_avg * 1e-3) / 1e9 if dom_avg > 0 else 0.0
-    step_gbs = ALG_BYTES_PER_DUALPOL_SAMPLE * units_per_step / (ms_per_step * 1e-3) / 1e9
+    step_gbs = alg_bytes_per_unit * units_per_step / (ms_per_step * 1e-3) / 1e9
     roofline = {
         "bound": "hbm", "kernel": dom_name, "achieved": achieved, "peak": peak, "unit": "GB/s",
         "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
@@ -297,7 +301,7 @@ def main():
                "d2h_bytes_per_step": int(out_bytes), "steps": k_e2e, "checksum": int(pin_out.view(-1)[::4099].to(torch.int32).sum())}
 
     cpu_baseline = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and args.sample_bits == 10:
         import oracle
         t0 = time.perf_counter()
         oracle.process(w.packed, w.A, w.n, w.T, w.P, w.weights, w.S, coarse=w.coarse, fine_delay=w.fine_delay,

@@ -151,7 +151,10 @@ int fengine_debug_fir(fengine_t *fe, const void *in, float *g_out, int64_t n_spe
  * equal coarse delays), "fused" (0/1, default 0: run the pol-packed path as ONE persistent kernel whose FIR -> FFT
  * transposition goes through an L2-resident ring of scratch slots instead of a full-size HBM scratch; T = 4, 8, 16),
  * "ring_slots" / "lag" (ring depth D and FIR-to-FFT phase distance of the fused kernel, D >= lag + 2 is enforced),
- * "fused_ctas_per_sm" (0 = occupancy), "host_chunks" (pieces of the fengine_process_host pipeline, 1 = no overlap).  Returns INVALID_ARG for
+ * "fused_ctas_per_sm" (0 = occupancy), "host_chunks" (pieces of the fengine_process_host pipeline, 1 = no overlap),
+ * "sample_bits" (4, 8, 10 (default), 12, 16: width of the packed input samples, same big-endian bit stream, sample u
+ * in bits [b u, b u + b); the stream is then L*b/8 bytes.  The paper's bit-depth sweep.  Widths other
+ * than 10 run the tiled kernels on the pol-packed path with 16 taps, else the generic kernels).  Returns INVALID_ARG for
  * unknown keys. */
 int fengine_set_option(fengine_t *fe, const char *key, int64_t value);
 

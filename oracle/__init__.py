@@ -8,6 +8,7 @@ from .oracle import (  # noqa: F401
     build,
     lib,
     unpack10,
+    unpack_bits,
     channelize_f64,
     process,
     direct_channel,

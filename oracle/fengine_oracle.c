@@ -12,6 +12,7 @@
  *
  * Pins (tests/test_oracle_pins.py, all `-m "not gpu"`):
  *   oracle_unpack10      P1  hand example + independent bit-by-bit packer round trip
+ *   oracle_unpack_bits   P1b every code of 4/8/12/16-bit samples through an independent packer; b = 10 == oracle_unpack10
  *   oracle_window/fir    P2  impulse response, T=1 block FFT; P3 delay == input shift
  *   oracle_fft_radix2    P4  O(N^2) DFT, on-bin tone, Parseval (P6)
  *   whole path           P5  closed form for a tone (DTFT of h), P7, P8, P10, P12
@@ -54,6 +55,22 @@ void oracle_unpack10(const uint8_t *bytes, int64_t n_samples, int16_t *out)
 {
     for (int64_t u = 0; u < n_samples; ++u)
         out[u] = (int16_t)unpack_one(bytes, u);
+}
+
+/* Other input bit depths (the paper's bit-depth sweep: "4, 8, 12 and 16-bit samples"): the same
+ * convention as R1 with b bits per sample: big-endian bit stream, sample u in bits [b*u, b*u + b), MSB first, two's
+ * complement.  Written bit by bit on purpose (no word tricks): b in 1..16. */
+void oracle_unpack_bits(const uint8_t *bytes, int64_t n_samples, int bits, int16_t *out)
+{
+    for (int64_t u = 0; u < n_samples; ++u) {
+        int v = 0;
+        for (int i = 0; i < bits; ++i) {
+            const int64_t bit = (int64_t)bits * u + i;
+            v = (v << 1) | ((bytes[bit >> 3] >> (7 - (int)(bit & 7))) & 1);
+        }
+        if (v & (1 << (bits - 1))) v -= 1 << bits;      /* sign-extend */
+        out[u] = (int16_t)v;
+    }
 }
 
 /* ---------------------------------------------------------------------------

@@ -80,6 +80,18 @@ def unpack10(packed: np.ndarray, n_samples: int) -> np.ndarray:
     return out
 
 
+def unpack_bits(packed: np.ndarray, n_samples: int, bits: int) -> np.ndarray:
+    """b-bit two's complement samples, MSB first (PAPER.md:273-279 bit-depth sweep; convention of R1)."""
+    packed = np.ascontiguousarray(packed, dtype=np.uint8)
+    assert 1 <= bits <= 16 and packed.size * 8 >= n_samples * bits
+    out = np.empty(n_samples, dtype=np.int16)
+    L = lib()
+    L.oracle_unpack_bits.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_void_p]
+    L.oracle_unpack_bits.restype = None
+    L.oracle_unpack_bits(_ptr(packed), n_samples, bits, _ptr(out))
+    return out
+
+
 def window(s: np.ndarray, N: int, T: int, m: int, c: int) -> np.ndarray:
     s = np.ascontiguousarray(s, dtype=np.float64)
     x = np.empty(N * T, dtype=np.float64)

@@ -136,10 +136,12 @@ class FEngine:
 
     def set_option(self, key: str, value: int):
         self._check(self._lib.fengine_set_option(self._h, key.encode(), int(value)))
+        if key == "sample_bits":
+            self.sample_bits = int(value)
 
     # -- sizes ----------------------------------------------------------------------------------
     def input_bytes(self, n_spectra: int) -> int:
-        return self.A * self.P * (self.N * (n_spectra + self.T - 1) // 4 * 5)
+        return self.A * self.P * (self.N * (n_spectra + self.T - 1) * getattr(self, "sample_bits", 10) // 8)
 
     def output_shape(self, n_spectra: int):
         return (self.A, n_spectra, self.n, self.P, 2)

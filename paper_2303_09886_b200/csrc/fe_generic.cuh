@@ -8,16 +8,20 @@
 
 namespace fe {
 
-// sample u of a packed stream (big-endian bit stream), 0 outside [0, L)
-__device__ __forceinline__ int gen_sample(const uint8_t *s, int64_t L, int64_t u)
+// sample u of a packed stream of `bits`-bit two's complement samples (big-endian bit stream, 10 bits in
+// the paper's deployment, 4..16 in its bit-depth sweep PAPER.md:273-279), 0 outside [0, L)
+__device__ __forceinline__ int gen_sample(const uint8_t *s, int64_t L, int64_t u, int bits)
 {
     if (u < 0 || u >= L) return 0;
-    const int64_t bit = 10 * u;
-    const uint8_t *b = s + (bit >> 3);
+    const int64_t bit = (int64_t)bits * u, nbytes = (L * bits) >> 3;
+    const int64_t B = bit >> 3;
     const int off = (int)(bit & 7);
-    const uint32_t w = ((uint32_t)b[0] << 8) | (uint32_t)b[1];      // 16-bit window holding the 10 bits
-    const int v = (int)((w >> (6 - off)) & 0x3FFu);
-    return (v ^ 512) - 512;
+    uint32_t w = (uint32_t)s[B] << 16;                               // 24-bit window holding the sample
+    if (B + 1 < nbytes) w |= (uint32_t)s[B + 1] << 8;
+    if (B + 2 < nbytes) w |= (uint32_t)s[B + 2];
+    const int v = (int)((w >> (24 - off - bits)) & ((1u << bits) - 1u));
+    const int sign = 1 << (bits - 1);
+    return (v ^ sign) - sign;
 }
 
 struct GenParams {
@@ -29,6 +33,7 @@ struct GenParams {
     int64_t n_coarse, n_fine;
     int64_t stream_bytes, L, n_spectra;
     int N, T, P, A;
+    int bits;                 // sample width of the packed input
 };
 
 // debug: window samples [A][P][S][N*T] int16
@@ -42,7 +47,7 @@ __global__ void gen_unpack_kernel(const GenParams p, int16_t *out)
         const int64_t m = (idx / NT) % p.n_spectra;
         const int64_t st = idx / NT / p.n_spectra;
         const int64_t c = p.coarse[st * p.n_coarse + (p.n_coarse == 1 ? 0 : m)];
-        out[idx] = (int16_t)gen_sample(p.in + st * p.stream_bytes, p.L, (int64_t)p.N * m - c + i);
+        out[idx] = (int16_t)gen_sample(p.in + st * p.stream_bytes, p.L, (int64_t)p.N * m - c + i, p.bits);
     }
 }
 
@@ -60,7 +65,7 @@ __global__ void gen_fir_kernel(const GenParams p, float *g)
         float acc = 0.f;
         for (int j = 0; j < p.T; ++j) {
             const int64_t u = (int64_t)p.N * (m + j) - c + t;
-            acc = fmaf((float)gen_sample(s, p.L, u), p.weights[t + (int64_t)p.N * j], acc);
+            acc = fmaf((float)gen_sample(s, p.L, u, p.bits), p.weights[t + (int64_t)p.N * j], acc);
         }
         g[idx] = acc;
     }

@@ -21,6 +21,7 @@
 #include "fe_fft2.cuh"
 #include "fe_fir.cuh"
 #include "fe_fir2.cuh"
+#include "fe_fir2b.cuh"
 #include "fe_fir3.cuh"
 #include "fe_fused.cuh"
 #include "fe_generic.cuh"
@@ -61,6 +62,7 @@ struct fengine {
     int lag = 5;                    // option "lag" (phases between a unit's FIR and FFT tasks)
     int fused_ctas_per_sm = 0;      // option "fused_ctas_per_sm" (0 = occupancy)
     int n_sms = 0;
+    int bits = 10;                  // option "sample_bits": width of the packed input samples (4, 8, 10, 12, 16)
     bool rg_dirty = true;
     // staging for fengine_process_host
     uint8_t *d_stage_in = nullptr;
@@ -179,10 +181,16 @@ int launch_fft2_n(fengine *fe, const Fft2Params &prm, int64_t chunk_len, cudaStr
 }
 
 // T = 32 exists only as the one-column pol-packed FIR (fe_fir3.cuh); other 32-tap engines run the generic kernels
-bool use_tiled(const fengine *fe) { return fe->tiled && (fe->T != 32 || use_packed(fe)); }
+// ... and sample widths other than 10 bits only as the 16-tap pol-packed FIR (fe_fir2.cuh)
+bool use_tiled(const fengine *fe)
+{
+    if (!fe->tiled) return false;
+    if (fe->bits != 10) return use_packed(fe) && fe->T == 16;
+    return fe->T != 32 || use_packed(fe);
+}
 bool use_fused(const fengine *fe)
 {
-    return use_packed(fe) && fe->allow_fused && fe->n <= 4096 && (fe->T == 4 || fe->T == 8 || fe->T == 16);
+    return use_packed(fe) && fe->allow_fused && fe->bits == 10 && fe->n <= 4096 && (fe->T == 4 || fe->T == 8 || fe->T == 16);
 }
 
 template <int T, class Plan, bool F32OUT>
@@ -272,6 +280,16 @@ int launch_fir2(fengine *fe, const Fir2Params &prm, int64_t chunk_len, cudaStrea
     }
     dim3 grid((unsigned)(fe->n / kFir2Threads), (unsigned)((chunk_len + prm.rows_per_tile - 1) / prm.rows_per_tile),
               (unsigned)fe->A);
+    if (fe->bits != 10) {                                   // bit-depth sweep: 16 taps only
+        switch (fe->bits) {
+        case 4: fir2b_kernel<16, 4><<<grid, kFir2Threads, 0, stream>>>(prm); break;
+        case 8: fir2b_kernel<16, 8><<<grid, kFir2Threads, 0, stream>>>(prm); break;
+        case 12: fir2b_kernel<16, 12><<<grid, kFir2Threads, 0, stream>>>(prm); break;
+        case 16: fir2b_kernel<16, 16><<<grid, kFir2Threads, 0, stream>>>(prm); break;
+        default: return fail(fe, FENGINE_ERR_INVALID_ARG, "no tiled FIR for %d-bit samples", fe->bits);
+        }
+        return FENGINE_OK;
+    }
     switch (fe->T) {
     case 2: fir2_kernel<2><<<grid, kFir2Threads, 0, stream>>>(prm); break;
     case 4: fir2_kernel<4><<<grid, kFir2Threads, 0, stream>>>(prm); break;
@@ -368,7 +386,8 @@ GenParams gen_params(const fengine *fe, const void *in, int64_t S)
     g.n_coarse = fe->n_coarse;
     g.n_fine = fe->n_fine;
     g.L = (int64_t)fe->N * (S + fe->T - 1);
-    g.stream_bytes = g.L / 4 * 5;
+    g.stream_bytes = g.L / 8 * fe->bits;
+    g.bits = fe->bits;
     g.n_spectra = S;
     g.N = fe->N;
     g.T = fe->T;
@@ -446,7 +465,7 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
     fp.coarse = fe->d_coarse;
     fp.n_coarse = fe->n_coarse;
     fp.rows_in = S + fe->T - 1;
-    fp.stream_bytes = (int64_t)fe->N * fp.rows_in / 4 * 5;
+    fp.stream_bytes = (int64_t)fe->N * fp.rows_in / 8 * fe->bits;
     fp.chunk_cap = chunk;
     fp.lgN = fe->lgN;
     fp.P = fe->P;
@@ -823,7 +842,7 @@ int fengine_process_host(fengine_t *fe, const void *in_host, void *out_host, int
     if (n_spectra < 0) return fail(fe, FENGINE_ERR_INVALID_ARG, "n_spectra < 0");
     if (n_spectra == 0) return FENGINE_OK;
     if (!in_host || !out_host) return fail(fe, FENGINE_ERR_INVALID_ARG, "null host pointer");
-    const size_t in_bytes = (size_t)fe->A * fe->P * ((size_t)fe->N * (n_spectra + fe->T - 1) / 4 * 5);
+    const size_t in_bytes = (size_t)fe->A * fe->P * ((size_t)fe->N * (n_spectra + fe->T - 1) / 8 * fe->bits);
     const size_t out_bytes = (size_t)fe->A * n_spectra * fe->n * fe->P * 2;
     if (!fe->host_stream) FE_CUDA(fe, cudaStreamCreateWithFlags(&fe->host_stream, cudaStreamNonBlocking));
     if (in_bytes > fe->stage_in_bytes) {
@@ -854,7 +873,7 @@ int fengine_process_host(fengine_t *fe, const void *in_host, void *out_host, int
     const int K = fe->host_chunks;
     if (use_tiled(fe) && !use_fused(fe) && K > 1 && n_spectra >= 4 * (int64_t)K) {
         const int64_t S = n_spectra, rows_in = S + fe->T - 1;
-        const size_t row_bytes = (size_t)fe->N / 4 * 5, stream_bytes = row_bytes * rows_in;
+        const size_t row_bytes = (size_t)fe->N / 8 * fe->bits, stream_bytes = row_bytes * rows_in;
         const int n_streams = fe->A * fe->P;
         const size_t out_row = (size_t)fe->n * fe->P * 2, out_pitch = out_row * S;
         if (!fe->s_h2d) FE_CUDA(fe, cudaStreamCreateWithFlags(&fe->s_h2d, cudaStreamNonBlocking));
@@ -943,7 +962,7 @@ int fengine_debug_fir(fengine_t *fe, const void *in, float *g_out, int64_t n_spe
         fp.coarse = fe->d_coarse;
         fp.n_coarse = fe->n_coarse;
         fp.rows_in = n_spectra + fe->T - 1;
-        fp.stream_bytes = (int64_t)fe->N * fp.rows_in / 4 * 5;
+        fp.stream_bytes = (int64_t)fe->N * fp.rows_in / 8 * fe->bits;
         fp.m_begin = 0;
         fp.m_end = n_spectra;
         fp.chunk_cap = n_spectra;
@@ -963,7 +982,7 @@ int fengine_debug_fir(fengine_t *fe, const void *in, float *g_out, int64_t n_spe
         fp.coarse = fe->d_coarse;
         fp.n_coarse = fe->n_coarse;
         fp.rows_in = n_spectra + fe->T - 1;
-        fp.stream_bytes = (int64_t)fe->N * fp.rows_in / 4 * 5;
+        fp.stream_bytes = (int64_t)fe->N * fp.rows_in / 8 * fe->bits;
         fp.m_begin = 0;
         fp.m_end = n_spectra;
         fp.chunk_cap = n_spectra;
@@ -1006,6 +1025,12 @@ int fengine_set_option(fengine_t *fe, const char *key, int64_t value)
     if (!strcmp(key, "host_chunks")) {
         if (value < 1 || value > 1024) return fail(fe, FENGINE_ERR_INVALID_ARG, "host_chunks out of range");
         fe->host_chunks = (int)value;
+        return FENGINE_OK;
+    }
+    if (!strcmp(key, "sample_bits")) {
+        if (value != 4 && value != 8 && value != 10 && value != 12 && value != 16)
+            return fail(fe, FENGINE_ERR_INVALID_ARG, "sample_bits must be 4, 8, 10, 12 or 16");
+        fe->bits = (int)value;
         return FENGINE_OK;
     }
     if (!strcmp(key, "fused")) {

@@ -14,7 +14,7 @@ from dataclasses import dataclass, field
 
 import numpy as np
 
-__all__ = ["pack10", "pack10_bitwise", "hann_sinc_weights", "Workload", "make_workload", "custom_workload",
+__all__ = ["pack10", "pack_bits", "pack10_bitwise", "hann_sinc_weights", "Workload", "make_workload", "custom_workload",
            "CONFIG_SHAPES"]
 
 
@@ -39,6 +39,33 @@ def pack10(samples: np.ndarray) -> np.ndarray:
         out[:, :, byte0] |= (w >> 8).astype(np.uint8)
         out[:, :, byte0 + 1] |= (w & 0xFF).astype(np.uint8)
     return out.reshape(*lead, L // 4 * 5)
+
+
+def pack_bits(samples: np.ndarray, bits: int) -> np.ndarray:
+    """Pack int samples (last axis) as `bits`-bit two's complement, MSB first (the convention of pack10; the
+    bit-depth sweep of PAPER.md:273-279 uses 4, 8, 12 and 16 bits).  length * bits must be a multiple of 8."""
+    s = np.asarray(samples)
+    L = s.shape[-1]
+    assert 1 <= bits <= 16 and (L * bits) % 8 == 0
+    assert s.min(initial=0) >= -(1 << (bits - 1)) and s.max(initial=0) <= (1 << (bits - 1)) - 1
+    if bits == 10:
+        return pack10(s)
+    lead = s.shape[:-1]
+    v = (s.astype(np.int32) & ((1 << bits) - 1)).astype(np.uint32).reshape(-1, L)
+    if bits == 8:
+        out = v.astype(np.uint8)
+    elif bits == 16:
+        out = np.stack([(v >> 8).astype(np.uint8), (v & 0xFF).astype(np.uint8)], axis=-1).reshape(v.shape[0], -1)
+    elif bits == 4:
+        out = ((v[:, 0::2] << 4) | v[:, 1::2]).astype(np.uint8)
+    elif bits == 12:
+        a, b = v[:, 0::2], v[:, 1::2]
+        out = np.stack([(a >> 4).astype(np.uint8), (((a & 15) << 4) | (b >> 8)).astype(np.uint8),
+                        (b & 0xFF).astype(np.uint8)], axis=-1).reshape(v.shape[0], -1)
+    else:
+        bitsarr = ((v[:, :, None] >> np.arange(bits - 1, -1, -1)) & 1).astype(np.uint8).reshape(v.shape[0], -1)
+        out = np.packbits(bitsarr, axis=-1)
+    return out.reshape(*lead, L * bits // 8)
 
 
 def pack10_bitwise(samples) -> np.ndarray:
@@ -103,8 +130,8 @@ class Workload:
         return self.N * (self.S + self.T - 1)
 
 
-def _samples(rng, L, N, sigma, tones):
-    """clip(rint(sigma * N(0,1) + sum A_i cos(2 pi k_i u / N + theta_i)), -512, 511); tones are on-bin."""
+def _samples(rng, L, N, sigma, tones, bits: int = 10):
+    """clip(rint(sigma * N(0,1) + sum A_i cos(2 pi k_i u / N + theta_i)), -2^(b-1), 2^(b-1) - 1); tones are on-bin."""
     x = rng.standard_normal(L, dtype=np.float32)
     x *= np.float32(sigma)
     if tones:
@@ -115,7 +142,7 @@ def _samples(rng, L, N, sigma, tones):
         reps = -(-L // N)
         x += np.tile(period.astype(np.float32), reps)[:L]
     np.rint(x, out=x)
-    np.clip(x, -512, 511, out=x)
+    np.clip(x, -(1 << (bits - 1)), (1 << (bits - 1)) - 1, out=x)
     return x.astype(np.int16)
 
 
@@ -127,12 +154,14 @@ def _random_gains(prng, A, P, n):
 
 def make_workload(config: int, n_spectra: int | None = None, n_antennas: int | None = None,
                   n_channels: int | None = None, seed: int = 0, keep_samples: bool = False,
-                  sigma: float | None = None, taps: int | None = None) -> Workload:
+                  sigma: float | None = None, taps: int | None = None, bits: int = 10) -> Workload:
     """Build the synthetic stand-in for BASELINE.json config `config` (1..5).
 
     n_spectra / n_antennas shrink the batch (same distributions) so that the oracle finishes in
     seconds; n_channels selects the sweep point of config 5.  `sigma` overrides the noise level
-    (config 4 variant 4b uses sigma=182, R17).  `taps` overrides T (the paper's tap sweep).
+    (config 4 variant 4b uses sigma=182, R17).  `taps` overrides T (the paper's tap sweep); `bits` != 10 packs
+    the samples at another width (bit-depth sweep) with sigma and tone amplitudes scaled by
+    2^(bits - 10), so that the signal fills the range the same way.
     """
     shp = dict(CONFIG_SHAPES[config])
     A = n_antennas or shp["A"]
@@ -186,25 +215,28 @@ def make_workload(config: int, n_spectra: int | None = None, n_antennas: int | N
     else:
         raise ValueError(config)
 
-    packed = np.empty((A, P, L // 4 * 5), dtype=np.uint8)
+    scale = 2.0 ** (bits - 10)
+    packed = np.empty((A, P, L * bits // 8), dtype=np.uint8)
     samples = np.empty((A, P, L), dtype=np.int16) if keep_samples else None
     for a in range(A):
         for p in range(P):
             rng = np.random.default_rng([seed, config, a, p])
-            s = _samples(rng, L, N, sig, tones[a])       # tone common to both pols, independent noise
-            packed[a, p] = pack10(s)
+            tn = tones[a] if bits == 10 else [(k, amp * scale, th) for (k, amp, th) in tones[a]]
+            s = _samples(rng, L, N, sig * scale, tn, bits)      # tone common to both pols, independent noise
+            packed[a, p] = pack_bits(s, bits)
             if keep_samples:
                 samples[a, p] = s
     return Workload(name=f"config{config}", A=A, P=P, n=n, T=T, S=S, packed=packed, weights=weights,
                     coarse=np.ascontiguousarray(coarse), fine_delay=np.ascontiguousarray(fine),
                     phase=np.ascontiguousarray(phase), gains=gains, samples=samples,
-                    meta=dict(config=config, sigma=sig, tones=tones, seed=seed))
+                    meta=dict(config=config, sigma=sig, tones=tones, seed=seed, bits=bits))
 
 
 def custom_workload(A: int, n: int, T: int, S: int, P: int = 2, seed: int = 0, sigma: float = 32.0,
                     coarse_range: tuple[int, int] | None = None, per_spectrum: bool = False,
-                    random_weights: bool = False, keep_samples: bool = True, tag: int = 99) -> Workload:
-    """Small free-form workload for edge-case parity tests (tiny n, odd T, negative delays, ...)."""
+                    random_weights: bool = False, keep_samples: bool = True, tag: int = 99, bits: int = 10) -> Workload:
+    """Small free-form workload for edge-case parity tests (tiny n, odd T, negative delays, ...).  `bits` != 10
+    packs the samples at another depth (sigma is the caller's business; the range is clipped to `bits`)."""
     N = 2 * n
     L = N * (S + T - 1)
     prng = np.random.default_rng([seed, tag, 10 ** 6, A, n, T, S])
@@ -218,16 +250,16 @@ def custom_workload(A: int, n: int, T: int, S: int, P: int = 2, seed: int = 0, s
     fine = prng.uniform(-0.5, 0.5, size=(A, P, nper)).astype(np.float32)
     phase = prng.uniform(0, 2 * np.pi, size=(A, P, nper)).astype(np.float32)
     gains = _random_gains(prng, A, P, n)
-    packed = np.empty((A, P, L // 4 * 5), dtype=np.uint8)
+    packed = np.empty((A, P, L * bits // 8), dtype=np.uint8)
     samples = np.empty((A, P, L), dtype=np.int16) if keep_samples else None
     for a in range(A):
         for p in range(P):
             rng = np.random.default_rng([seed, tag, a, p, n, S])
             k = int(rng.integers(1, max(n, 2)))
-            s = _samples(rng, L, N, sigma, [(k, 2 * sigma, float(rng.random()))])
-            packed[a, p] = pack10(s)
+            s = _samples(rng, L, N, sigma, [(k, 2 * sigma, float(rng.random()))], bits)
+            packed[a, p] = pack_bits(s, bits)
             if keep_samples:
                 samples[a, p] = s
     return Workload(name=f"custom_A{A}_n{n}_T{T}_S{S}", A=A, P=P, n=n, T=T, S=S, packed=packed,
                     weights=weights, coarse=coarse, fine_delay=fine, phase=phase, gains=gains,
-                    samples=samples, meta=dict(seed=seed, sigma=sigma))
+                    samples=samples, meta=dict(seed=seed, sigma=sigma, bits=bits))

@@ -245,6 +245,39 @@ def test_32_taps(torch, fb, n, S, A, per_spectrum, equal_pols):
     check_parity(got, oracle_run(w), f"T=32 n={n}")
 
 
+@pytest.mark.parametrize("bits,n,T,S,equal_pols", [
+    (8, 1024, 16, 70, True), (16, 4096, 16, 40, True), (12, 2048, 16, 45, True), (4, 1024, 16, 33, True),
+    (12, 8192, 16, 20, True),
+    (8, 64, 5, 9, False), (16, 32, 3, 7, False),                 # generic kernels
+])
+def test_other_sample_widths(torch, fb, bits, n, T, S, equal_pols):
+    """4 / 8 / 12 / 16-bit input, option sample_bits: unpack bit-exact, whole path vs the oracle."""
+    sigma = {4: 2.0, 8: 30.0, 12: 400.0, 16: 6000.0}[bits]
+    w = si.custom_workload(A=2, n=n, T=T, S=S, P=2, seed=59, bits=bits, sigma=sigma, coarse_range=(-n, 3 * n),
+                           random_weights=(n <= 64))
+    if equal_pols:
+        w.coarse[:, 1] = w.coarse[:, 0]
+    for a in range(w.A):                                         # the packed stream decodes to the kept samples
+        for p in range(w.P):
+            np.testing.assert_array_equal(oracle.unpack_bits(w.packed[a, p], w.L, bits), w.samples[a, p])
+    fe = make_engine(fb, w, sample_bits=bits)
+    d_in = torch.from_numpy(w.packed.reshape(-1)).cuda()
+    if n <= 64:                                                  # steps 1-2 bit-exact through the debug hook
+        d_win = torch.zeros((w.A, w.P, S, w.N * T), dtype=torch.int16, device="cuda")
+        fe.debug_unpack(d_in, d_win, S)
+        torch.cuda.synchronize()
+        win = d_win.cpu().numpy()
+        for a in range(w.A):
+            for p in range(w.P):
+                for m in range(S):
+                    ref = oracle.window(w.samples[a, p].astype(np.float64), w.N, T, m, int(w.coarse[a, p, 0]))
+                    np.testing.assert_array_equal(win[a, p, m], ref.astype(np.int16))
+    got = gpu_run(torch, fe, w)
+    ref = oracle.channelize_f64(w.samples, w.n, w.T, w.weights, coarse=w.coarse, fine_delay=w.fine_delay,
+                                phase=w.phase, gains=w.gains, n_spectra=S)
+    check_parity(got, ref, f"{bits}-bit n={n}")
+
+
 def test_generic_and_tiled_kernels_agree(torch, fb):
     w = si.make_workload(1, n_spectra=6)
     a = gpu_run(torch, make_engine(fb, w), w)

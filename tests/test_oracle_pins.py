@@ -375,3 +375,35 @@ def test_selection_of_spectra_matches_full_run():
                           fine_delay=w.fine_delay, phase=w.phase, gains=w.gains, sel=sel)
     np.testing.assert_array_equal(part["Y"], full["Y"][:, sel])
     np.testing.assert_array_equal(part["out"], full["out"][:, sel])
+
+
+# ---------------------------------------------------------------------------------------------
+# P1b  other sample widths (PAPER.md:273-279 bit-depth sweep): same bit-stream convention as R1
+# ---------------------------------------------------------------------------------------------
+def _pack_strings(values, bits):
+    """Independent packer: binary strings, no shifts shared with oracle or generators."""
+    stream = "".join(format(int(v) & ((1 << bits) - 1), f"0{bits}b") for v in values)
+    assert len(stream) % 8 == 0
+    return np.array([int(stream[i:i + 8], 2) for i in range(0, len(stream), 8)], dtype=np.uint8)
+
+
+@pytest.mark.parametrize("bits", [4, 8, 10, 12, 16])
+def test_unpack_bits_every_code_round_trips(bits):
+    lo, hi = -(1 << (bits - 1)), (1 << (bits - 1)) - 1
+    codes = np.arange(lo, hi + 1, dtype=np.int64)
+    rng = np.random.default_rng(bits)
+    codes = np.concatenate([codes, rng.integers(lo, hi + 1, size=64)])       # and a shuffled tail
+    got = oracle.unpack_bits(_pack_strings(codes, bits), codes.size, bits)
+    np.testing.assert_array_equal(got.astype(np.int64), codes)
+    np.testing.assert_array_equal(si.pack_bits(codes, bits), _pack_strings(codes, bits))   # the generator's packer too
+
+
+def test_unpack_bits_at_10_bits_is_unpack10_and_hand_examples():
+    rng = np.random.default_rng(3)
+    s = rng.integers(-512, 512, size=256)
+    pk = si.pack10(s)
+    np.testing.assert_array_equal(oracle.unpack_bits(pk, s.size, 10), oracle.unpack10(pk, s.size))
+    # hand examples: 4-bit [1, -1, 7, -8] = 0x1F 0x78; 12-bit [1, -1] = 0x00 0x1F 0xFF; 16-bit [-2] = 0xFF 0xFE
+    np.testing.assert_array_equal(oracle.unpack_bits(np.array([0x1F, 0x78], np.uint8), 4, 4), [1, -1, 7, -8])
+    np.testing.assert_array_equal(oracle.unpack_bits(np.array([0x00, 0x1F, 0xFF], np.uint8), 2, 12), [1, -1])
+    np.testing.assert_array_equal(oracle.unpack_bits(np.array([0xFF, 0xFE], np.uint8), 1, 16), [-2])
