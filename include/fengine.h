@@ -127,6 +127,28 @@ int fengine_process_host(fengine_t *fe, const void *in_host, void *out_host, int
  */
 int fengine_process_heaps(fengine_t *fe, const void *in, void *heaps_out, int64_t n_spectra, void *stream);
 
+/*
+ * Streaming (the input is processed in chunks and the samples a chunk's last spectra still need
+ * are carried over to the next chunk; coarse delays reach outside the chunk).  Between
+ * fengine_stream_begin and fengine_stream_end consecutive fengine_stream_push calls continue ONE sample stream per
+ * (antenna, pol): every call supplies the next n_new rows of N samples and returns n_new spectra; the handle keeps
+ * the rows that later windows still need in a device window buffer (two buffers, tail copied device to device).
+ *
+ * fengine_stream_begin   sizes the history from the coarse delays set so far: D = T - 1 + ceil(max(-c, 0) / N) rows of
+ *                        latency (written to *delay_out if non-null) and ceil(max(c, 0) / N) + 1 further rows of
+ *                        history; max_new_spectra bounds n_new of every push.  Samples before the first push are 0.
+ * fengine_stream_push    in_new: DEVICE, 16-byte aligned, [A][P][n_new * N * bits / 8] bytes (the new rows only);
+ *                        out: DEVICE [A][n_new][n][P][2] int8.  Output j of the push is spectrum G + j - D of the
+ *                        stream, G = rows pushed before this call: the concatenated outputs of all pushes equal
+ *                        fengine_process on [D zero rows, then the whole stream] (same coarse delays), which is what
+ *                        the tests check.  Delay tables with n_per_stream > 1 are indexed by j.  Coarse delays set
+ *                        during a stream must not need more history than begin kept (FENGINE_ERR_STATE).
+ * fengine_stream_end     closes the stream; fengine_process is refused while one is open.
+ */
+int fengine_stream_begin(fengine_t *fe, int64_t max_new_spectra, int64_t *delay_out);
+int fengine_stream_push(fengine_t *fe, const void *in_new, void *out, int64_t n_new, void *stream);
+int fengine_stream_end(fengine_t *fe);
+
 /* Human-readable description of the last error on this handle ("" if none). */
 const char *fengine_last_error(const fengine_t *fe);
 

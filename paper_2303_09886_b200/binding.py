@@ -16,6 +16,7 @@ EXPORTED_SYMBOLS = [
     "fengine_set_fine_delays", "fengine_set_gains", "fengine_process", "fengine_process_host",
     "fengine_last_error", "fengine_process_f32", "fengine_debug_unpack", "fengine_debug_fir",
     "fengine_set_option", "fengine_last_launch_count", "fengine_profile_read", "fengine_process_heaps",
+    "fengine_stream_begin", "fengine_stream_push", "fengine_stream_end",
 ]
 
 STATUS = {0: "OK", 1: "INVALID_ARG", 2: "ALLOC", 3: "CUDA", 4: "STATE"}
@@ -53,6 +54,9 @@ def lib() -> C.CDLL:
         L.fengine_process.argtypes = [vp, vp, vp, i64, vp]
         L.fengine_process_host.argtypes = [vp, vp, vp, i64]
         L.fengine_process_heaps.argtypes = [vp, vp, vp, i64, vp]
+        L.fengine_stream_begin.argtypes = [vp, i64, vp]
+        L.fengine_stream_push.argtypes = [vp, vp, vp, i64, vp]
+        L.fengine_stream_end.argtypes = [vp]
         L.fengine_process_f32.argtypes = [vp, vp, vp, i64, vp]
         L.fengine_debug_unpack.argtypes = [vp, vp, vp, i64, vp]
         L.fengine_debug_fir.argtypes = [vp, vp, vp, i64, vp]
@@ -158,6 +162,18 @@ class FEngine:
         """fengine_process_heaps: channel-major heaps of 256 spectra (int8, shape heaps_shape(n_spectra))."""
         self._check(self._lib.fengine_process_heaps(self._h, _dev_ptr(inp), _dev_ptr(heaps_out), n_spectra,
                                                     _stream_handle(stream)))
+
+    def stream_begin(self, max_new_spectra: int) -> int:
+        """fengine_stream_begin; returns the latency D in spectra."""
+        d = C.c_int64(0)
+        self._check(self._lib.fengine_stream_begin(self._h, max_new_spectra, C.byref(d)))
+        return int(d.value)
+
+    def stream_push(self, inp_new, out, n_new: int, stream=None):
+        self._check(self._lib.fengine_stream_push(self._h, _dev_ptr(inp_new), _dev_ptr(out), n_new, _stream_handle(stream)))
+
+    def stream_end(self):
+        self._check(self._lib.fengine_stream_end(self._h))
 
     def process_f32(self, inp, out_f32, n_spectra: int, stream=None):
         self._check(self._lib.fengine_process_f32(self._h, _dev_ptr(inp), _dev_ptr(out_f32), n_spectra,

@@ -62,6 +62,14 @@ struct fengine {
     int lag = 5;                    // option "lag" (phases between a unit's FIR and FFT tasks)
     int fused_ctas_per_sm = 0;      // option "fused_ctas_per_sm" (0 = occupancy)
     int n_sms = 0;
+    // streaming (fengine_stream_*): user coarse delays, row offset folded into the device table, window buffers
+    std::vector<int32_t> h_coarse;
+    int64_t stream_off = 0;         // rows the device table is shifted by (0 = not streaming)
+    int64_t rows_override = 0;      // rows per stream of the buffer given to process_impl (0 = S + T - 1)
+    uint8_t *d_win[2] = {nullptr, nullptr};
+    size_t win_bytes = 0;
+    int64_t win_H = 0, win_max_new = 0, win_prev_new = 0, win_delay = 0;
+    int win_cur = 0;
     int bits = 10;                  // option "sample_bits": width of the packed input samples (4, 8, 10, 12, 16)
     bool rg_dirty = true;
     // staging for fengine_process_host
@@ -385,7 +393,7 @@ GenParams gen_params(const fengine *fe, const void *in, int64_t S)
     g.gains = fe->d_gains;
     g.n_coarse = fe->n_coarse;
     g.n_fine = fe->n_fine;
-    g.L = (int64_t)fe->N * (S + fe->T - 1);
+    g.L = (int64_t)fe->N * (fe->rows_override > 0 ? fe->rows_override : S + fe->T - 1);
     g.stream_bytes = g.L / 8 * fe->bits;
     g.bits = fe->bits;
     g.n_spectra = S;
@@ -464,7 +472,7 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
     fp.g = fe->d_scratch;
     fp.coarse = fe->d_coarse;
     fp.n_coarse = fe->n_coarse;
-    fp.rows_in = S + fe->T - 1;
+    fp.rows_in = fe->rows_override > 0 ? fe->rows_override : S + fe->T - 1;
     fp.stream_bytes = (int64_t)fe->N * fp.rows_in / 8 * fe->bits;
     fp.chunk_cap = chunk;
     fp.lgN = fe->lgN;
@@ -704,6 +712,8 @@ void fengine_destroy(fengine_t *fe)
     cudaFree(fe->d_scratch);
     cudaFree(fe->d_ring);
     cudaFree(fe->d_ctl);
+    cudaFree(fe->d_win[0]);
+    cudaFree(fe->d_win[1]);
     cudaFree(fe->d_rec);
     cudaFree(fe->d_stage_in);
     cudaFree(fe->d_stage_out);
@@ -734,7 +744,14 @@ int fengine_set_coarse_delays(fengine_t *fe, const int32_t *c, int64_t n_per_str
         fe->d_coarse = nd;
         fe->n_coarse = n_per_stream;
     }
-    FE_CUDA(fe, cudaMemcpy(fe->d_coarse, c, sizeof(int32_t) * count, cudaMemcpyHostToDevice));
+    fe->h_coarse.assign(c, c + count);
+    if (fe->stream_off != 0) {                              // streaming: the row offset of the window lives in the table
+        std::vector<int32_t> eff(count);
+        for (size_t i = 0; i < count; ++i) eff[i] = (int32_t)((int64_t)c[i] - fe->stream_off * fe->N);
+        FE_CUDA(fe, cudaMemcpy(fe->d_coarse, eff.data(), sizeof(int32_t) * count, cudaMemcpyHostToDevice));
+    } else {
+        FE_CUDA(fe, cudaMemcpy(fe->d_coarse, c, sizeof(int32_t) * count, cudaMemcpyHostToDevice));
+    }
     fe->c_min = fe->c_max = c[0];
     for (size_t i = 1; i < count; ++i) {
         fe->c_min = std::min(fe->c_min, c[i]);
@@ -797,6 +814,7 @@ int fengine_process(fengine_t *fe, const void *in, void *out, int64_t n_spectra,
 {
     int rc = check_call(fe, in, out, n_spectra);
     if (rc) return rc;
+    if (fe->stream_off != 0) return fail(fe, FENGINE_ERR_STATE, "a stream is open: use fengine_stream_push or fengine_stream_end");
     return process_impl(fe, in, static_cast<int8_t *>(out), nullptr, n_spectra, static_cast<cudaStream_t>(stream));
 }
 
@@ -833,6 +851,96 @@ int fengine_process_heaps(fengine_t *fe, const void *in, void *heaps_out, int64_
     ++fe->last_launches;
     FE_CUDA(fe, cudaGetLastError());
     return FENGINE_OK;
+}
+
+// ---- streaming: consecutive pushes continue one sample stream -------------------------------
+namespace {
+int64_t ceil_div_rows(int64_t x, int lgN) { return x <= 0 ? 0 : (x + ((int64_t)1 << lgN) - 1) >> lgN; }
+
+int upload_coarse(fengine *fe)
+{
+    const size_t count = (size_t)fe->A * fe->P * fe->n_coarse;
+    std::vector<int32_t> eff(count, 0);
+    for (size_t i = 0; i < count; ++i)
+        eff[i] = (int32_t)((int64_t)(i < fe->h_coarse.size() ? fe->h_coarse[i] : 0) - fe->stream_off * fe->N);
+    FE_CUDA(fe, cudaMemcpy(fe->d_coarse, eff.data(), sizeof(int32_t) * count, cudaMemcpyHostToDevice));
+    return FENGINE_OK;
+}
+}  // namespace
+
+int fengine_stream_begin(fengine_t *fe, int64_t max_new_spectra, int64_t *delay_out)
+{
+    if (!fe) return FENGINE_ERR_INVALID_ARG;
+    fe->err.clear();
+    if (max_new_spectra < 1) return fail(fe, FENGINE_ERR_INVALID_ARG, "max_new_spectra < 1");
+    FE_CUDA(fe, cudaDeviceSynchronize());
+    const int64_t back = ceil_div_rows(fe->c_max, fe->lgN) + 1;       // rows a positive delay (and a lagging column) reach back
+    const int64_t fwd = ceil_div_rows(-(int64_t)fe->c_min, fe->lgN);  // rows a negative delay reaches ahead
+    fe->win_delay = fe->T - 1 + fwd;
+    fe->win_H = fe->win_delay + back;
+    fe->win_max_new = max_new_spectra;
+    const size_t row_bytes = (size_t)fe->N / 8 * fe->bits;
+    const size_t bytes = (size_t)fe->A * fe->P * (size_t)(fe->win_H + max_new_spectra) * row_bytes;
+    if (bytes > fe->win_bytes) {
+        for (auto &w : fe->d_win) {
+            cudaFree(w);
+            w = nullptr;
+        }
+        fe->win_bytes = 0;
+        for (auto &w : fe->d_win)
+            if (cudaMalloc(&w, bytes) != cudaSuccess) {
+                cudaGetLastError();
+                return fail(fe, FENGINE_ERR_ALLOC, "cannot allocate %zu bytes for the stream window", bytes);
+            }
+        fe->win_bytes = bytes;
+    }
+    FE_CUDA(fe, cudaMemset(fe->d_win[0], 0, fe->win_bytes));         // samples before the stream started are 0 (R3)
+    fe->win_cur = 0;
+    fe->win_prev_new = 0;
+    fe->stream_off = back;
+    int rc = upload_coarse(fe);
+    if (rc) return rc;
+    fe->rg_dirty = true;
+    fe->rg2_mode = -1;
+    if (delay_out) *delay_out = fe->win_delay;
+    return FENGINE_OK;
+}
+
+int fengine_stream_push(fengine_t *fe, const void *in_new, void *out, int64_t n_new, void *stream)
+{
+    int rc = check_call(fe, in_new, out, n_new);
+    if (rc || n_new == 0) return rc;
+    if (fe->stream_off == 0) return fail(fe, FENGINE_ERR_STATE, "no stream is open (fengine_stream_begin)");
+    if (n_new > fe->win_max_new) return fail(fe, FENGINE_ERR_INVALID_ARG, "more spectra than fengine_stream_begin allowed");
+    if (ceil_div_rows(fe->c_max, fe->lgN) + 1 > fe->stream_off || fe->T - 1 + ceil_div_rows(-(int64_t)fe->c_min, fe->lgN) > fe->win_delay)
+        return fail(fe, FENGINE_ERR_STATE, "coarse delays set after fengine_stream_begin need more history than it kept");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const size_t rb = (size_t)fe->N / 8 * fe->bits;
+    const int n_streams = fe->A * fe->P;
+    const int nxt = fe->win_cur ^ 1;
+    const size_t pitch_prev = (size_t)(fe->win_H + fe->win_prev_new) * rb, pitch_new = (size_t)(fe->win_H + n_new) * rb;
+    // the last H rows of the previous window, then the new rows (the overlap-tail copy of PAPER.md:85-87)
+    FE_CUDA(fe, cudaMemcpy2DAsync(fe->d_win[nxt], pitch_new, fe->d_win[fe->win_cur] + (size_t)fe->win_prev_new * rb, pitch_prev,
+                                  (size_t)fe->win_H * rb, n_streams, cudaMemcpyDeviceToDevice, s));
+    FE_CUDA(fe, cudaMemcpy2DAsync(fe->d_win[nxt] + (size_t)fe->win_H * rb, pitch_new, in_new, (size_t)n_new * rb,
+                                  (size_t)n_new * rb, n_streams, cudaMemcpyDeviceToDevice, s));
+    fe->rows_override = fe->win_H + n_new;
+    rc = process_impl(fe, fe->d_win[nxt], static_cast<int8_t *>(out), nullptr, n_new, s);
+    fe->rows_override = 0;
+    fe->win_cur = nxt;
+    fe->win_prev_new = n_new;
+    return rc;
+}
+
+int fengine_stream_end(fengine_t *fe)
+{
+    if (!fe) return FENGINE_ERR_INVALID_ARG;
+    fe->err.clear();
+    FE_CUDA(fe, cudaDeviceSynchronize());
+    fe->stream_off = 0;
+    fe->rg_dirty = true;
+    fe->rg2_mode = -1;
+    return upload_coarse(fe);
 }
 
 int fengine_process_host(fengine_t *fe, const void *in_host, void *out_host, int64_t n_spectra)

@@ -278,6 +278,54 @@ def test_other_sample_widths(torch, fb, bits, n, T, S, equal_pols):
     check_parity(got, ref, f"{bits}-bit n={n}")
 
 
+@pytest.mark.parametrize("n,T,A,crange,pushes,equal_pols", [
+    (1024, 16, 2, (0, 1), [40, 17, 64, 1, 30], True),            # no delay: history = T - 1 rows (+1)
+    (1024, 16, 2, (-3000, 5000), [40, 17, 64], True),            # windows reach back and ahead of the chunk
+    (4096, 8, 1, (-20000, 9000), [33, 90], False),               # unequal pols: one-pol kernels
+    (64, 3, 2, (-200, 300), [5, 9, 2], False),                   # generic kernels
+])
+def test_streaming_pushes_equal_one_batch(torch, fb, n, T, A, crange, pushes, equal_pols):
+    """fengine_stream_*: concatenated pushes == fengine_process on [D zero rows, stream]."""
+    R = sum(pushes)
+    N = 2 * n
+    w = si.custom_workload(A=A, n=n, T=T, S=R - (T - 1), P=2, seed=61, coarse_range=crange, random_weights=(n <= 64))
+    if equal_pols:
+        w.coarse[:, 1] = w.coarse[:, 0]
+    rows = w.packed.reshape(A, 2, R, N // 4 * 5)                  # the stream, row by row
+    fe = make_engine(fb, w)
+    D = fe.stream_begin(max(pushes))
+    c = w.coarse.reshape(-1)
+    assert D == T - 1 + max(0, -(-max(0, -int(c.min())) // N))
+    outs, r0 = [], 0
+    for k in pushes:
+        d_new = torch.from_numpy(np.ascontiguousarray(rows[:, :, r0:r0 + k]).reshape(-1)).cuda()
+        d_out = torch.full(fe.output_shape(k), 99, dtype=torch.int8, device="cuda")
+        fe.stream_push(d_new, d_out, k)
+        torch.cuda.synchronize()
+        outs.append(d_out.cpu().numpy())
+        r0 += k
+    with pytest.raises(fb.FEngineError):
+        fe.process(d_new, d_out, 1)                               # refused while a stream is open
+    fe.stream_end()
+    got = np.concatenate(outs, axis=1)                            # [A][R][n][P][2]
+    # the same thing as one batch: D zero rows in front, T - 1 zero rows behind so that R spectra exist
+    padded = np.zeros((A, 2, D + R + T - 1, N // 4 * 5), np.uint8)
+    padded[:, :, D:D + R] = rows
+    S2 = D + R
+    d_in = torch.from_numpy(padded.reshape(-1)).cuda()
+    d_out = torch.zeros(fe.output_shape(S2), dtype=torch.int8, device="cuda")
+    fe.process(d_in, d_out, S2)
+    torch.cuda.synchronize()
+    batch = d_out.cpu().numpy()[:, :R]
+    # spectra whose window lies inside what has been pushed agree exactly; the last ones of the batch see the zero
+    # padding instead of rows that a later push would have delivered, as the stream does at its end
+    np.testing.assert_array_equal(got, batch)
+    ref = oracle.process(padded, A, n, T, 2, w.weights, S2, coarse=w.coarse, fine_delay=w.fine_delay, phase=w.phase,
+                         gains=w.gains, want_Y=False)["out"][:, :R]
+    diff = np.abs(got.astype(np.int32) - ref.astype(np.int32))
+    assert diff.max() <= 1 and np.count_nonzero(diff) <= max(2, int(1e-4 * diff.size))
+
+
 def test_generic_and_tiled_kernels_agree(torch, fb):
     w = si.make_workload(1, n_spectra=6)
     a = gpu_run(torch, make_engine(fb, w), w)
