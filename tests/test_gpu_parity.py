@@ -326,6 +326,41 @@ def test_streaming_pushes_equal_one_batch(torch, fb, n, T, A, crange, pushes, eq
     assert diff.max() <= 1 and np.count_nonzero(diff) <= max(2, int(1e-4 * diff.size))
 
 
+def test_fp32_fft_has_no_spurs_with_a_dithered_tone(torch, fb):
+    """The paper's precision gate (Fig. 6): a tone in channel 192 of 1024, quantised to 10 bits
+    with uniform dither, transformed many times and averaged in double precision.  An FP16 FFT shows harmonics near
+    -75 dB there; the FP32 path of this library must stay at the averaging floor."""
+    n, N, K, k0, amp = 1024, 2048, 4096, 192, 200.0
+    rng = np.random.default_rng(67)
+    u = np.arange(N)
+    tone = amp * np.cos(2 * np.pi * k0 * u / N + 0.3)
+    s = np.floor(tone[None, :] + rng.random((K, N))).astype(np.int16)         # uniform dither, 10-bit range
+    assert s.min() >= -512 and s.max() <= 511
+    flat = np.concatenate([s.reshape(-1), np.zeros(N, np.int16)])             # T = 2 needs one more row (unused: tap 1 is 0)
+    packed = si.pack10(flat)[None, None, :]
+    packed = np.concatenate([packed, packed], axis=1)                         # both pols carry the same stream
+    h = np.concatenate([np.ones(N, np.float32), np.zeros(N, np.float32)])     # tap 0 = 1, tap 1 = 0: the path is the plain
+    fe = fb.FEngine(n, 2, 2, h, n_antennas=1)                                 # FFT of every row, on the tiled kernels
+    d_in = torch.from_numpy(np.ascontiguousarray(packed).reshape(-1)).cuda()
+    d_y = torch.zeros(fe.output_shape(K), dtype=torch.float32, device="cuda")
+    fe.process_f32(d_in, d_y, K)
+    torch.cuda.synchronize()
+    y = d_y[0, :, :, 0].to(torch.float64).mean(dim=0).cpu().numpy()          # average over the K transforms
+    avg = y[:, 0] + 1j * y[:, 1]
+    p_db = 10 * np.log10(np.maximum(np.abs(avg) ** 2, 1e-300) / np.abs(avg[k0]) ** 2)
+    assert abs(abs(avg[k0]) - amp * N / 2) < 1e-3 * amp * N / 2
+    others = np.delete(p_db, k0)
+    # averaging floor: dither noise (1/12 per sample) summed over N samples, averaged over K transforms
+    floor_db = 10 * np.log10((N / 12.0 / K) / (amp * N / 2) ** 2)
+    assert floor_db < -105
+    assert others.max() < floor_db + 13, (others.max(), floor_db)              # nothing sticks out of the noise floor
+    assert others.max() < -95                                                  # far below the FP16 harmonics (-75 dB)
+    # and the float64 oracle averages to the same spectrum
+    ref = oracle.channelize_f64(np.stack([flat, flat])[None].astype(np.float64), n, 2, h,
+                                n_spectra=K)["Y"][0, :, :, 0].mean(axis=0)
+    assert np.abs(avg - ref).max() < 1e-6 * abs(ref[k0])
+
+
 def test_generic_and_tiled_kernels_agree(torch, fb):
     w = si.make_workload(1, n_spectra=6)
     a = gpu_run(torch, make_engine(fb, w), w)
