@@ -163,6 +163,10 @@ struct SpectrumPhase2 {      // shared, filled once per spectrum in per-spectrum
     float4 step[16];         // exp(-2 pi i d_eff Q kq / N)
     float4 c3;               // exp(2 i phi) exp(-i pi d_eff): E[n-k] = c3 * conj(E[k]) with E incl. exp(i phi)
     float4 ephi;             // exp(i phi)
+    // E(k0) of a thread's first channel k0 = h + SW (K_lo + 16 K_hi) as a product of two table words, so that the
+    // double-precision sincos runs 80 times per spectrum (here) instead of twice per thread and sweep
+    float4 lo[2][16];        // [sweep h][K_lo]: exp(i phi) exp(-2 pi i d_eff (h + SW K_lo) / N)
+    float4 hi[16];           // [K_hi]: exp(-2 pi i d_eff 16 SW K_hi / N)
 };
 
 __device__ __forceinline__ cx<f2> unpack_unit(float4 v) { return {f2(v.x, v.y), f2(v.z, v.w)}; }
@@ -242,22 +246,7 @@ __device__ __forceinline__ void fft2_pass3(float4 *sm, const Fft2Params &prm, in
     // per-thread rotation base of the per-spectrum mode: E_p(K) = exp(i phi_p) exp(-2 pi i (d_p + cr) K / N)
     cx<f2> base = {f2(1.f, 1.f), f2(0.f, 0.f)};
     const float4 *__restrict__ gtab = reinterpret_cast<const float4 *>(prm.rg2) + (int64_t)a * n;
-    if (prm.per_spectrum) {
-        float2 e[2];
-#pragma unroll
-        for (int p = 0; p < 2; ++p) {
-            const int64_t st = (int64_t)a * 2 + p;
-            const int32_t c = prm.coarse[st * prm.n_coarse + (prm.n_coarse == 1 ? 0 : m)];
-            const int cr = (int)(c & (N - 1));
-            const double d = (double)prm.fine_d[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
-            const double phi = (double)prm.fine_phi[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
-            const double t = -(d / (double)N) * (double)k0 - (double)((cr * k0) & (N - 1)) / (double)N;
-            double sp_, cp_;
-            sincos(phi, &sp_, &cp_);
-            e[p] = cmulf(phasor_turns(t), make_float2((float)cp_, (float)sp_));
-        }
-        base = {f2(e[0].x, e[1].x), f2(e[0].y, e[1].y)};
-    }
+    if (prm.per_spectrum) base = cmul2(unpack_unit(sph->lo[HS][K & 15]), unpack_unit(sph->hi[K >> 4]));
     // post-twiddle phasors without a table walk: (sin, cos)(2 pi (K + Q kq) / N) = the thread's own (sin, cos)(2 pi K / N)
     // rotated by the compile-time angle 2 pi kq Q / N (Q / N is 1/32 or 1/16), one table word per thread and spectrum
     const float2 tpK = __ldg(prm.tpost + k0);
@@ -318,33 +307,39 @@ __device__ __forceinline__ void fft2_setup_phase(const Fft2Params &prm, Spectrum
 {
     constexpr int N = 2 * Plan::n;
     const int p = tid >> 5, t = tid & 31;
-    if (p < 2 && t <= 16) {
+    if (p < 2) {                                          // warp p sets up pol p: every lane a few phasors in double
         const int64_t st = (int64_t)a * 2 + p;
         const int32_t c = prm.coarse[st * prm.n_coarse + (prm.n_coarse == 1 ? 0 : m)];
         const int cr = (int)(c & (N - 1));
         const double d = (double)prm.fine_d[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
         const double phi = (double)prm.fine_phi[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
-        if (t < 16) {
-            const int k = Plan::SW * Plan::Q * t;
-            const double tt = -(d / (double)N) * (double)k - (double)((cr * k) & (N - 1)) / (double)N;
-            const float2 v = phasor_turns(tt);
-            float *dst = reinterpret_cast<float *>(&sph->step[t]);
+        auto phasor = [&](int k) {                        // exp(-2 pi i (d + cr) k / N), the cr part reduced exactly
+            return phasor_turns(-(d / (double)N) * (double)k - (double)((cr * k) & (N - 1)) / (double)N);
+        };
+        auto put = [&](float4 *dst4, float2 v) {
+            float *dst = reinterpret_cast<float *>(dst4);
             dst[p] = v.x;
             dst[2 + p] = v.y;
+        };
+        double sphi, cphi;
+        sincos(phi, &sphi, &cphi);
+        const float2 ephi = make_float2((float)cphi, (float)sphi);
+        if (t < 16) {
+            put(&sph->step[t], phasor(Plan::SW * Plan::Q * t));
+            put(&sph->lo[0][t], cmulf(phasor(Plan::SW * t), ephi));
         } else {
+            const int j = t - 16;
+            put(&sph->hi[j], phasor(16 * Plan::SW * j));
+            put(&sph->lo[1][j], cmulf(phasor(1 + Plan::SW * j), ephi));
+        }
+        if (t == 16) {
+            put(&sph->ephi, ephi);
             double s, c_;
-            sincos(phi, &s, &c_);
-            float *de = reinterpret_cast<float *>(&sph->ephi);
-            de[p] = (float)c_;
-            de[2 + p] = (float)s;
             sincos(2.0 * phi, &s, &c_);
             const float2 e2 = make_float2((float)c_, (float)s);
-            float2 h = phasor_turns(-0.5 * d);        // exp(-i pi d_eff) = exp(-i pi d) * (-1)^cr
+            float2 h = phasor_turns(-0.5 * d);            // exp(-i pi d_eff) = exp(-i pi d) * (-1)^cr
             if (cr & 1) { h.x = -h.x; h.y = -h.y; }
-            const float2 c3 = cmulf(e2, h);
-            float *dc = reinterpret_cast<float *>(&sph->c3);
-            dc[p] = c3.x;
-            dc[2 + p] = c3.y;
+            put(&sph->c3, cmulf(e2, h));
         }
     }
 }
