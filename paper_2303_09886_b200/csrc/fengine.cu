@@ -822,6 +822,7 @@ int fengine_process_heaps(fengine_t *fe, const void *in, void *heaps_out, int64_
 {
     int rc = check_call(fe, in, heaps_out, n_spectra);
     if (rc || n_spectra == 0) return rc;
+    if (fe->stream_off != 0) return fail(fe, FENGINE_ERR_STATE, "a stream is open: use fengine_stream_push or fengine_stream_end");
     if (fe->n < 32) return fail(fe, FENGINE_ERR_INVALID_ARG, "heaps need n >= 32");
     const size_t bytes = (size_t)fe->A * n_spectra * fe->n * fe->P * 2;
     if (bytes > fe->rec_bytes) {
@@ -950,6 +951,7 @@ int fengine_process_host(fengine_t *fe, const void *in_host, void *out_host, int
     if (n_spectra < 0) return fail(fe, FENGINE_ERR_INVALID_ARG, "n_spectra < 0");
     if (n_spectra == 0) return FENGINE_OK;
     if (!in_host || !out_host) return fail(fe, FENGINE_ERR_INVALID_ARG, "null host pointer");
+    if (fe->stream_off != 0) return fail(fe, FENGINE_ERR_STATE, "a stream is open: use fengine_stream_push or fengine_stream_end");
     const size_t in_bytes = (size_t)fe->A * fe->P * ((size_t)fe->N * (n_spectra + fe->T - 1) / 8 * fe->bits);
     const size_t out_bytes = (size_t)fe->A * n_spectra * fe->n * fe->P * 2;
     if (!fe->host_stream) FE_CUDA(fe, cudaStreamCreateWithFlags(&fe->host_stream, cudaStreamNonBlocking));
@@ -1038,6 +1040,7 @@ int fengine_process_f32(fengine_t *fe, const void *in, float *spectra_out, int64
 {
     int rc = check_call(fe, in, spectra_out, n_spectra);
     if (rc) return rc;
+    if (fe->stream_off != 0) return fail(fe, FENGINE_ERR_STATE, "a stream is open: use fengine_stream_push or fengine_stream_end");
     return process_impl(fe, in, nullptr, spectra_out, n_spectra, static_cast<cudaStream_t>(stream));
 }
 
