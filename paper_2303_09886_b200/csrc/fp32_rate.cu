@@ -1,4 +1,4 @@
-// fp32_rate.cu -- FP32 issue-rate microbenchmark for sm_100a (not part of the library).
+// fp32_rate.cu -- FP32 issue-rate (and legacy mma.sync rate) microbenchmark for sm_100a (not part of the library).
 //
 // Measures how many FP32 lane-operations per clock per SM the FMA pipe sustains for the instruction forms the
 // F-engine kernels use (packed FFMA2 / FADD2 / FMUL2, scalar FFMA), with and without operand reuse.
@@ -63,6 +63,24 @@ void run(const char *name, int threads, int ctas_per_sm)
     printf("%-28s threads=%4d ctas/sm=%d  %.3f ms  %.1f lane-ops/clk/SM (at 1.965 GHz)  %.2f T lane-ops/s\n", name, threads, ctas_per_sm, ms, per_clk_sm, lane_ops / (ms * 1e-3) / 1e12);
     cudaFree(out);
 }
+// legacy tensor path: mma.sync.m16n8k16 f16 x f16 + f32 (what a tensor-core FIR would use)
+__global__ void k_hmma(float *out, unsigned a0)
+{
+    unsigned a[4] = {a0 + threadIdx.x, a0 ^ 0x3c003c00u, a0 + 7, a0 + 9};
+    unsigned b[2] = {0x3c003c00u, 0x38003800u};
+    float d[8][4];
+    for (int i = 0; i < 8; ++i) for (int j = 0; j < 4; ++j) d[i][j] = 0.f;
+    for (int it = 0; it < ITERS; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+            asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                         : "+f"(d[i][0]), "+f"(d[i][1]), "+f"(d[i][2]), "+f"(d[i][3])
+                         : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
+    }
+    float r = 0;
+    for (int i = 0; i < 8; ++i) for (int j = 0; j < 4; ++j) r += d[i][j];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = r;
+}
 int main()
 {
     for (int t : {128, 256, 512, 1024}) {
@@ -73,6 +91,25 @@ int main()
         run<4>("FMUL2 const", t, 1);
         run<5>("FFMA2 acc*s+acc", t, 1);
         run<7>("FFMA2 s0*bcast+pair (reuse)", t, 1);
+    }
+    {
+        float *out;
+        cudaMalloc(&out, 148 * 1024 * 4 * sizeof(float));
+        for (int threads : {128, 256, 512, 1024}) {
+            cudaEvent_t e0, e1;
+            cudaEventCreate(&e0); cudaEventCreate(&e1);
+            k_hmma<<<148, threads>>>(out, 0x3c00u);
+            cudaDeviceSynchronize();
+            cudaEventRecord(e0);
+            for (int r = 0; r < 5; ++r) k_hmma<<<148, threads>>>(out, 0x3c00u);
+            cudaEventRecord(e1);
+            cudaEventSynchronize(e1);
+            float ms; cudaEventElapsedTime(&ms, e0, e1); ms /= 5;
+            const double mmas = 148.0 * (threads / 32) * ITERS * 8;
+            printf("mma.sync m16n8k16 f16        threads=%4d ctas/sm=1  %.3f ms  %.1f TFLOP/s  %.2f cycles per HMMA per SMSP (at 1.965 GHz)\n",
+                   threads, ms, mmas * 2.0 * 16 * 8 * 16 / (ms * 1e-3) / 1e12, (ms * 1e-3 * 1.965e9) / (ITERS * 8.0 * (threads / 32) / 4.0));
+        }
+        cudaFree(out);
     }
     return 0;
 }
