@@ -272,12 +272,12 @@ def main():
     roofline["fused"] = bool(n_fir and fir_avg < 0.02 * max(fft_avg, 1e-9))
     if roofline["fused"]:
         roofline["kernel"] = dom_name = "fused_kernel"
-    prof = ROOT / "profiles" / "roofline_traffic.json"
+    prof = ROOT / "profiles" / "roofline_traffic.csv"       # ncu dram bytes per launch of the committed capture
     if prof.exists():
-        try:
-            roofline["traffic"] = json.loads(prof.read_text()).get(dom_name)
-        except Exception:
-            pass
+        for ln in prof.read_text().splitlines():
+            parts = ln.split(",")
+            if len(parts) == 2 and parts[0] == dom_name and parts[1].isdigit():
+                roofline["traffic"] = int(parts[1])
 
     # ---- end to end through fengine_process_host: pinned host buffers, H2D + path + D2H per step ----
     e2e = None
