@@ -103,6 +103,16 @@ int fengine_set_gains(fengine_t *fe, const float *gains_re_im);
 int fengine_process(fengine_t *fe, const void *in, void *out, int64_t n_spectra, void *stream);
 
 /*
+ * fengine_reserve -- size every buffer fengine_process needs for calls of up to max_spectra spectra (SURVEY.md 8(b):
+ * "the library never allocates in this call").  Without a reserve the first fengine_process call, and any call larger
+ * than all before it, allocates (and synchronises the device once); after a successful reserve fengine_process never
+ * allocates, never synchronises, and can be captured in a CUDA graph: a call that would need more returns
+ * FENGINE_ERR_STATE.  The reserve is made for the kernels the handle would run now (options, equal or unequal
+ * coarse delays of the two pols); call it again after changing those.  Off the hot path: synchronises the device.
+ */
+int fengine_reserve(fengine_t *fe, int64_t max_spectra);
+
+/*
  * fengine_process_host -- the same path for HOST buffers (the paper's regime: input chunks arrive
  * in pinned host memory and results go back to the host).
  * in_host / out_host  HOST pointers (pinned or pageable), same layouts as fengine_process.
@@ -191,6 +201,11 @@ int fengine_profile_read(fengine_t *fe, double *fir_ms, double *fft_ms, int64_t 
 
 /* Number of kernel launches the last fengine_process / _f32 call enqueued (for bench accounting). */
 int64_t fengine_last_launch_count(const fengine_t *fe);
+
+/* Test hook: with option "pipe_stats" = 1 the pipelined kernel accumulates 16 SM-clock counters per CTA (waits of its
+ * three roles, rows per team; layout in csrc/fe_pipe.cuh).  Copies up to max_words of them to HOST `out`
+ * ([n_sms][16] uint64) and zeroes them.  Synchronises the device. */
+int fengine_debug_pipe_stats(fengine_t *fe, uint64_t *out, int64_t max_words);
 
 #ifdef __cplusplus
 }

@@ -16,7 +16,7 @@ EXPORTED_SYMBOLS = [
     "fengine_set_fine_delays", "fengine_set_gains", "fengine_process", "fengine_process_host",
     "fengine_last_error", "fengine_process_f32", "fengine_debug_unpack", "fengine_debug_fir",
     "fengine_set_option", "fengine_last_launch_count", "fengine_profile_read", "fengine_process_heaps",
-    "fengine_stream_begin", "fengine_stream_push", "fengine_stream_end",
+    "fengine_stream_begin", "fengine_stream_push", "fengine_stream_end", "fengine_reserve", "fengine_debug_pipe_stats",
 ]
 
 STATUS = {0: "OK", 1: "INVALID_ARG", 2: "ALLOC", 3: "CUDA", 4: "STATE"}
@@ -53,6 +53,8 @@ def lib() -> C.CDLL:
         L.fengine_set_gains.argtypes = [vp, vp]
         L.fengine_process.argtypes = [vp, vp, vp, i64, vp]
         L.fengine_process_host.argtypes = [vp, vp, vp, i64]
+        L.fengine_reserve.argtypes = [vp, i64]
+        L.fengine_debug_pipe_stats.argtypes = [vp, vp, i64]
         L.fengine_process_heaps.argtypes = [vp, vp, vp, i64, vp]
         L.fengine_stream_begin.argtypes = [vp, i64, vp]
         L.fengine_stream_push.argtypes = [vp, vp, vp, i64, vp]
@@ -150,6 +152,10 @@ class FEngine:
     def output_shape(self, n_spectra: int):
         return (self.A, n_spectra, self.n, self.P, 2)
 
+    def reserve(self, max_spectra: int):
+        """fengine_reserve: size every buffer now so that process() never allocates."""
+        self._check(self._lib.fengine_reserve(self._h, int(max_spectra)))
+
     # -- the hot path -----------------------------------------------------------------------------
     def process(self, inp, out, n_spectra: int, stream=None):
         """fengine_process: device tensors (uint8 in, int8 out); asynchronous on `stream`."""
@@ -201,6 +207,12 @@ class FEngine:
         na, nb = C.c_int64(), C.c_int64()
         self._check(self._lib.fengine_profile_read(self._h, C.byref(a), C.byref(b), C.byref(na), C.byref(nb)))
         return a.value, b.value, na.value, nb.value
+
+    def pipe_stats(self, n_sms: int = 148):
+        """fengine_debug_pipe_stats: [n_sms][16] uint64 clock counters of the pipelined kernel (option pipe_stats)."""
+        out = np.zeros((n_sms, 16), dtype=np.uint64)
+        self._check(self._lib.fengine_debug_pipe_stats(self._h, _host_ptr(out), out.size))
+        return out
 
     def last_launch_count(self) -> int:
         return int(self._lib.fengine_last_launch_count(self._h))

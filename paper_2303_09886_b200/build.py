@@ -1,61 +1,70 @@
 """Build the CUDA shared library in-tree (sm_100a only).
 
-    python -m paper_2303_09886_b200.build [--force]
+    python -m paper_2303_09886_b200.build [--force] [-v]
 
-nvcc cross-compiles without a GPU.  The .so is git-ignored but travels with the tree.
+nvcc cross-compiles without a GPU.  Every csrc/*.cu is one translation unit; they compile in parallel and are linked
+into one shared library.  The .so is git-ignored but travels with the tree.
 """
 from __future__ import annotations
 
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 from pathlib import Path
 
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
+OBJ = PKG / "build"
 LIB = PKG / "libfengine_b200.so"
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-lineinfo", "-std=c++17",
-    "-shared", "-Xcompiler", "-fPIC",
+    "-Xcompiler", "-fPIC",
 ]
 
 
-def sources():
-    return sorted(CSRC.glob("*.cu")) + sorted(CSRC.glob("*.cuh")) + [PKG.parent / "include" / "fengine.h"]
+def units():
+    return sorted(CSRC.glob("*.cu"))
+
+
+def headers():
+    return sorted(CSRC.glob("*.cuh")) + [PKG.parent / "include" / "fengine.h"]
 
 
 def needs_build() -> bool:
     if not LIB.exists():
         return True
     t = LIB.stat().st_mtime
-    return any(s.stat().st_mtime > t for s in sources())
+    return any(s.stat().st_mtime > t for s in units() + headers())
 
 
 def build(force: bool = False, verbose: bool = False) -> Path:
     if not force and not needs_build():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    OBJ.mkdir(exist_ok=True)
+    hdr_time = max(h.stat().st_mtime for h in headers())
+
+    def compile_one(src: Path) -> Path:
+        obj = OBJ / (src.stem + ".o")
+        if not force and obj.exists() and obj.stat().st_mtime > max(src.stat().st_mtime, hdr_time):
+            return obj
+        cmd = [nvcc, *NVCC_FLAGS, "-c", "-o", str(obj), str(src)]
+        if verbose:
+            cmd.insert(1, "-Xptxas=-v")
+            print(" ".join(cmd), flush=True)
+        subprocess.check_call(cmd)
+        return obj
+
+    with ThreadPoolExecutor(max_workers=max(1, len(units()))) as ex:
+        objs = list(ex.map(compile_one, units()))
     tmp = LIB.with_suffix(f".so.tmp{os.getpid()}")
-    cmd = [nvcc, *NVCC_FLAGS, "-o", str(tmp), str(CSRC / "fengine.cu")]
-    if verbose:
-        cmd.insert(1, "-Xptxas=-v")
-        print(" ".join(cmd))
-    subprocess.check_call(cmd)
+    subprocess.check_call([nvcc, "-shared", "-o", str(tmp), *[str(o) for o in objs]])
     os.replace(tmp, LIB)
     return LIB
-
-
-def build_tools() -> Path:
-    """The FP32 issue-rate microbenchmark (csrc/fp32_rate.cu), a standalone program."""
-    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    exe = PKG / "fp32_rate"
-    subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", str(exe), str(CSRC / "fp32_rate.cu")])
-    return exe
 
 
 if __name__ == "__main__":
     build(force="--force" in sys.argv, verbose="-v" in sys.argv)
     print(LIB)
-    if "--tools" in sys.argv:
-        print(build_tools())

@@ -480,7 +480,7 @@ constexpr size_t fft_smem_bytes(int P)
 // exchange buffer (small CTAs, several per SM, each at a different phase of its spectrum).  A
 // two-sweep plan (n = 32768) runs the whole sequence once for the even and once for the odd channels.
 template <class Plan, bool F32OUT>
-__global__ void __launch_bounds__(Plan::tpf, (512 / Plan::tpf) > 0 ? (512 / Plan::tpf) : 1) fft_kernel(const FftParams prm)
+static __global__ void __launch_bounds__(Plan::tpf, (512 / Plan::tpf) > 0 ? (512 / Plan::tpf) : 1) fft_kernel(const FftParams prm)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int n = Plan::n, N = 2 * n, SW = Plan::sweeps;
@@ -573,7 +573,7 @@ __global__ void __launch_bounds__(Plan::tpf, (512 / Plan::tpf) > 0 ? (512 / Plan
 // table builders (device, float64 trigonometry; run once at create / when parameters change)
 // ------------------------------------------------------------------------------------------------
 // tw[k][lo] for one pass: W_M^{k tau'}, tau' = 2 lo, 2 lo + 1
-__global__ void build_pass_twiddles(float4 *tw, int R, int S, int M)
+static __global__ void build_pass_twiddles(float4 *tw, int R, int S, int M)
 {
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= R * S) return;
@@ -585,7 +585,7 @@ __global__ void build_pass_twiddles(float4 *tw, int R, int S, int M)
     tw[idx] = make_float4((float)c0, (float)c1, (float)s0, (float)s1);
 }
 
-__global__ void build_post_twiddles(float2 *tp, int n)
+static __global__ void build_post_twiddles(float2 *tp, int n)
 {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n) return;
@@ -595,7 +595,7 @@ __global__ void build_post_twiddles(float2 *tp, int n)
 }
 
 // const mode: rg[a][p][k] = 0.5 * G * exp(i(-2 pi (d + cr) k / N + phi))
-__global__ void build_rg_table(float2 *rg, const float2 *gains, const int32_t *coarse, const float *fine_d,
+static __global__ void build_rg_table(float2 *rg, const float2 *gains, const int32_t *coarse, const float *fine_d,
                                const float *fine_phi, int n, int n_streams)
 {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;

@@ -46,6 +46,21 @@ struct Fft2Plan {
 
 __device__ __forceinline__ cx<f2> unpack_unit_ld(float4 v) { return {f2(v.x, v.y), f2(v.z, v.w)}; }
 
+// Where pass 1 reads the row from: the scratch in global memory (two-kernel path, streamed past the L1) or a
+// shared-memory landing buffer that a bulk copy filled (pipelined kernel, fe_pipe.cuh).  operator()(i) = unit i.
+struct RowInGlobal {
+    const float4 *p;
+    __device__ __forceinline__ float4 operator()(int i) const { return ldg_stream_f4(p + i); }
+};
+struct RowInShared {
+    uint32_t s;                 // shared-space address of unit 0
+    __device__ __forceinline__ float4 operator()(int i) const { return lds_f4(s + (uint32_t)i * 16u); }
+};
+// CTA-wide barrier of the one-spectrum-per-CTA kernels; the pipelined kernel passes a named barrier over its FFT team
+struct SyncCta {
+    __device__ __forceinline__ void operator()() const { __syncthreads(); }
+};
+
 struct Fft2Params {
     const float *g;           // scratch rows a*chunk_cap + (m - m_begin), n units of 16 bytes
     int8_t *out;              // [A][S][n][2][2] or null
@@ -63,29 +78,29 @@ struct Fft2Params {
 };
 
 // top radix-2 stage of the radix-32 first digit, element J of sweep HS (compile-time J so that W_32^J is a constant)
-template <class Plan, int HS, int J>
-__device__ __forceinline__ void fft2_sweep_half(const float4 *__restrict__ grow, int col, cx<f2> (&a)[16])
+template <class Plan, int HS, int J, class Row>
+__device__ __forceinline__ void fft2_sweep_half(const Row &grow, int col, cx<f2> (&a)[16])
 {
     if constexpr (J < 16) {
-        const cx<f2> xu = unpack_unit_ld(ldg_stream_f4(grow + J * Plan::M1 + col));
-        const cx<f2> xv = unpack_unit_ld(ldg_stream_f4(grow + (J + 16) * Plan::M1 + col));
+        const cx<f2> xu = unpack_unit_ld(grow(J * Plan::M1 + col));
+        const cx<f2> xv = unpack_unit_ld(grow((J + 16) * Plan::M1 + col));
         if constexpr (HS == 0)
             a[J] = cadd(xu, xv);
         else
             a[J] = mul_w<32, J, f2>(csub(xu, xv));
-        fft2_sweep_half<Plan, HS, J + 1>(grow, col, a);
+        fft2_sweep_half<Plan, HS, J + 1, Row>(grow, col, a);
     }
 }
 
 // pass 1 of sweep HS of a two-sweep plan: outputs k1 = 2 k'' + HS, twiddle W_n^{k1 col} as a running product
-template <class Plan, int HS>
-__device__ __forceinline__ void fft2_pass1_sweep(const float4 *__restrict__ grow, float4 *sm, const float2 *__restrict__ tw, int tid)
+template <class Plan, int HS, class Row>
+__device__ __forceinline__ void fft2_pass1_sweep(const Row &grow, float4 *sm, const float2 *__restrict__ tw, int tid)
 {
     constexpr int M1 = Plan::M1;
     for (int col = tid; col < M1; col += Plan::tpf) {
         cx<f2> a[16];
         const float2 w1 = __ldg(tw + M1 + col);           // W_n^{col}
-        fft2_sweep_half<Plan, HS, 0>(grow, col, a);
+        fft2_sweep_half<Plan, HS, 0, Row>(grow, col, a);
         Dif<16, f2>::run(a);
         const float2 w2 = cmulf(w1, w1);
         float2 wk = HS ? w1 : w2;
@@ -101,15 +116,15 @@ __device__ __forceinline__ void fft2_pass1_sweep(const float4 *__restrict__ grow
     }
 }
 
-template <class Plan>
-__device__ __forceinline__ void fft2_pass1(const float4 *__restrict__ grow, float4 *sm, const float2 *__restrict__ tw, int tid)
+template <class Plan, class Row>
+__device__ __forceinline__ void fft2_pass1(const Row &grow, float4 *sm, const float2 *__restrict__ tw, int tid)
 {
     constexpr int R = Plan::R1, M1 = Plan::M1;
     for (int col = tid; col < M1; col += Plan::tpf) {
         cx<f2> x[R];
 #pragma unroll
         for (int t = 0; t < R; ++t) {
-            const float4 v = ldg_stream_f4(grow + t * M1 + col);
+            const float4 v = grow(t * M1 + col);
             x[t].re = f2(v.x, v.y);
             x[t].im = f2(v.z, v.w);
         }
@@ -217,9 +232,9 @@ __device__ __forceinline__ void fft2_epilogue(cx<f2> zk, cx<f2> zm, float2 tp, c
 // and also owns the self-mirrored channel n/2.
 // Two-sweep plans (HS = sweep): residue K of sweep HS holds the channels k = HS + SW (K + Q kq); in the odd sweep
 // the mirror of residue K is residue Q - 1 - K and no residue mirrors onto itself.
-template <class Plan, bool F32OUT, int HS = 0>
+template <class Plan, bool F32OUT, int HS, class Sync>
 __device__ __forceinline__ void fft2_pass3(float4 *sm, const Fft2Params &prm, int a, int64_t m, int tid,
-                                           const SpectrumPhase2 *sph)
+                                           const SpectrumPhase2 *sph, const Sync &sync)
 {
     constexpr int R = Plan::R3, H = R / 2, Q = Plan::Q, n = Plan::n, N = 2 * n, SW = Plan::SW;
     static_assert(Plan::tpf == Q, "one residue per thread");
@@ -283,7 +298,7 @@ __device__ __forceinline__ void fft2_pass3(float4 *sm, const Fft2Params &prm, in
         }
     };
 
-    __syncthreads();                                      // upper halves are in the exchange buffer
+    sync();                                               // upper halves are in the exchange buffer
 #pragma unroll
     for (int kq = 0; kq < H; ++kq) {
         const int kA = k0 + SW * Q * kq, kB = n - kA;      // kB == n for the DC channel (dropped Nyquist)
@@ -344,38 +359,36 @@ __device__ __forceinline__ void fft2_setup_phase(const Fft2Params &prm, Spectrum
     }
 }
 
-// One spectrum of one antenna, both pols, by the whole CTA.  `after_load()` runs (on every thread) once the
-// scratch row has been consumed (after the barrier that ends pass 1); the fused kernel releases the ring slot there.
-// `after_pass2()` runs after the barrier that ends pass 2 (the fused kernel samples its next task's dependency there).
-template <class Plan, bool F32OUT, class AfterLoad, class AfterPass2>
-__device__ __forceinline__ void fft2_row(const Fft2Params &prm, const float4 *grow, unsigned char *smem_raw, int a,
-                                         int64_t m, int tid, AfterLoad after_load, AfterPass2 after_pass2)
+// One spectrum of one antenna, both pols, by the tpf threads that share `sync` (the whole CTA, or the FFT team of
+// the pipelined kernel).  `after_load()` runs (on every thread) once the row has been consumed (after the barrier
+// that ends the last pass 1): the pipelined kernel hands its landing buffer back to the loader there.
+template <class Plan, bool F32OUT, class Row, class Sync, class AfterLoad>
+__device__ __forceinline__ void fft2_row(const Fft2Params &prm, const Row &grow, unsigned char *smem_raw, int a,
+                                         int64_t m, int tid, const Sync &sync, AfterLoad after_load)
 {
     float4 *sm = reinterpret_cast<float4 *>(smem_raw);
     SpectrumPhase2 *sph = reinterpret_cast<SpectrumPhase2 *>(smem_raw + (size_t)Plan::units * 16);
     if (prm.per_spectrum) fft2_setup_phase<Plan>(prm, sph, a, m, tid);
     if constexpr (Plan::SW == 1) {
         fft2_pass1<Plan>(grow, sm, prm.tw1, tid);
-        __syncthreads();
+        sync();
         after_load();
         fft2_pass2<Plan>(sm, prm.tw2, tid);
-        __syncthreads();
-        after_pass2();
-        fft2_pass3<Plan, F32OUT>(sm, prm, a, m, tid, sph);
+        sync();
+        fft2_pass3<Plan, F32OUT, 0>(sm, prm, a, m, tid, sph, sync);
     } else {
         fft2_pass1_sweep<Plan, 0>(grow, sm, prm.tw1, tid);
-        __syncthreads();
+        sync();
         fft2_pass2<Plan>(sm, prm.tw2, tid);
-        __syncthreads();
-        fft2_pass3<Plan, F32OUT, 0>(sm, prm, a, m, tid, sph);
-        __syncthreads();                                  // the exchange buffer is reused by the odd sweep
+        sync();
+        fft2_pass3<Plan, F32OUT, 0>(sm, prm, a, m, tid, sph, sync);
+        sync();                                           // the exchange buffer is reused by the odd sweep
         fft2_pass1_sweep<Plan, 1>(grow, sm, prm.tw1, tid);
-        __syncthreads();
+        sync();
         after_load();
         fft2_pass2<Plan>(sm, prm.tw2, tid);
-        __syncthreads();
-        after_pass2();
-        fft2_pass3<Plan, F32OUT, 1>(sm, prm, a, m, tid, sph);
+        sync();
+        fft2_pass3<Plan, F32OUT, 1>(sm, prm, a, m, tid, sph, sync);
     }
 }
 
@@ -387,7 +400,7 @@ constexpr size_t fft2_smem_bytes()
 
 // One CTA per (antenna, spectrum), both pols.
 template <class Plan, bool F32OUT>
-__global__ void __launch_bounds__(Plan::tpf, (512 / Plan::tpf) > 0 ? (512 / Plan::tpf) : 1) fft2_kernel(const Fft2Params prm)
+static __global__ void __launch_bounds__(Plan::tpf, (512 / Plan::tpf) > 0 ? (512 / Plan::tpf) : 1) fft2_kernel(const Fft2Params prm)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int N = 2 * Plan::n;
@@ -396,14 +409,14 @@ __global__ void __launch_bounds__(Plan::tpf, (512 / Plan::tpf) > 0 ? (512 / Plan
     const int a = (int)gridDim.y - 1 - (int)blockIdx.y;
     const int64_t m = prm.m_end - 1 - (int64_t)blockIdx.x;
     if (m < prm.m_begin) return;
-    const float4 *grow = reinterpret_cast<const float4 *>(prm.g + ((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * (int64_t)N * 2);
-    fft2_row<Plan, F32OUT>(prm, grow, smem_raw, a, m, threadIdx.x, [] {}, [] {});
+    const RowInGlobal grow{reinterpret_cast<const float4 *>(prm.g + ((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * (int64_t)N * 2)};
+    fft2_row<Plan, F32OUT>(prm, grow, smem_raw, a, m, threadIdx.x, SyncCta{}, [] {});
 }
 
 // Pol-interleaved table of the pol-packed epilogue, [A][n] units {re p0, re p1, im p0, im p1}:
 //   const mode          0.5 * G * exp(i(-2 pi (d + cr) k / N + phi))   (rotation folded in)
 //   per-spectrum mode   G                                              (rotation computed per spectrum in the kernel)
-__global__ void build_rg2_table(float4 *rg2, const float2 *gains, const int32_t *coarse, const float *fine_d,
+static __global__ void build_rg2_table(float4 *rg2, const float2 *gains, const int32_t *coarse, const float *fine_d,
                                 const float *fine_phi, int n, int A, int per_spectrum)
 {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
@@ -433,7 +446,7 @@ __global__ void build_rg2_table(float4 *rg2, const float2 *gains, const int32_t 
 }
 
 // scalar twiddle table of one pass: tw[k][x] = W_M^{k x} = (cos, -sin)(2 pi k x / M)
-__global__ void build_scalar_twiddles(float2 *tw, int R, int S, int M)
+static __global__ void build_scalar_twiddles(float2 *tw, int R, int S, int M)
 {
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= R * S) return;
@@ -444,7 +457,7 @@ __global__ void build_scalar_twiddles(float2 *tw, int R, int S, int M)
 }
 
 // debug: natural-order FIR output g [A][2][S][N] from pol-packed scratch rows (a*cap + m), undoing the rotation
-__global__ void unrotate2_kernel(const float *gp, float *g_out, const int32_t *coarse, int64_t n_coarse,
+static __global__ void unrotate2_kernel(const float *gp, float *g_out, const int32_t *coarse, int64_t n_coarse,
                                  int64_t n_spectra, int64_t cap, int N, int A)
 {
     const int64_t total = (int64_t)A * 2 * n_spectra * N;

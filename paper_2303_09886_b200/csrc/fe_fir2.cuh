@@ -38,15 +38,38 @@ constexpr int kFir2Warps = kFir2Threads / 32;
 constexpr int kFir2SegBytes = 80;                                   // per warp per row per pol: 16 groups x 5 bytes
 constexpr int kFir2SlotBytes = 2 * kFir2SegBytes;                   // both pols
 
+// Where the finished rows of a run go.  A sink sees, for every step s = 0, 1, .. of the run, one call of
+// store(cur) (the 16-byte unit of this thread's point for the run-relative row sp = s - T + lag, which the sink
+// counts itself and must ignore outside [0, n_out)), bracketed by before_steps(s) ahead of every 8th step and
+// after_steps(s) behind every 8th step (warp-uniform hooks: flow control and completion signalling of the
+// pipelined kernel, fe_pipe.cuh; empty here).
+struct Fir2ScratchSink {            // two-kernel path: rows of the linear scratch, one row per spectrum
+    float *gp;
+    size_t g_stride;
+    int sp, n_out;
+    __device__ __forceinline__ void begin_run(int lag, int T, int n_out_) { gp += ((int64_t)lag - T) * (int64_t)g_stride; sp = lag - T; n_out = n_out_; }
+    __device__ __forceinline__ void before_steps(int) {}
+    __device__ __forceinline__ void after_steps(int) {}
+    __device__ __forceinline__ void end_run() {}
+    __device__ __forceinline__ void store(float4 cur)
+    {
+        asm volatile("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %5, %6;\n\t@p st.global.v4.f32 [%0], {%1, %2, %3, %4};\n\t}"
+                     ::"l"(gp), "f"(cur.x), "f"(cur.y), "f"(cur.z), "f"(cur.w), "r"((unsigned)sp), "r"((unsigned)n_out) : "memory");
+        gp += g_stride;
+        ++sp;
+    }
+};
+
 // Ring step q holds input row R0 + q of both pols, R0 = m0 - cq - 1; see fir_run in fe_fir.cuh for the
 // partial-sum bookkeeping, which is identical.
-template <int T, bool MIXED>
+// NC: the row width N when the caller knows it at compile time (row strides become immediates), else 0.
+template <int T, bool MIXED, class Sink, int NC = 0>
 __device__ __forceinline__ void fir2_run(const Fir2Params &prm, const uint8_t *wsrc, uint32_t ring_s, int64_t c,
-                                         int64_t m0, int n_out, int i_pt, float *grow0)
+                                         int64_t m0, int n_out, int i_pt, Sink &sink)
 {
     constexpr int U = kFirUnroll;
     static_assert(U % T == 0 && U % kFirDepth == 0, "unroll must cover whole tap and ring periods");
-    const int N = 1 << prm.lgN;
+    const int N = NC ? NC : 1 << prm.lgN;
     const int lane = threadIdx.x & 31;
     const int cr = (int)(c & (int64_t)(N - 1));
     const int64_t cq = (c - cr) >> prm.lgN;
@@ -117,9 +140,7 @@ __device__ __forceinline__ void fir2_run(const Fir2Params &prm, const uint8_t *w
     for (int j = 0; j < T; ++j) acc0[j] = acc1[j] = f2(0.f, 0.f);
     float4 prev = make_float4(0.f, 0.f, 0.f, 0.f);
 
-    const size_t g_stride = (size_t)N * 2;                      // next spectrum (floats): n units of 4 floats
-    float *gp = grow0 + 4 * i_pt + ((int64_t)(MIXED ? 0 : lag0) - T) * (int64_t)g_stride;
-    int sp = (MIXED ? 0 : lag0) - T;
+    sink.begin_run(MIXED ? 0 : lag0, T, n_out);
 
     // The loop is software-pipelined by one step and has no branch in its unrolled body: the raw words of step
     // ii + 1 are read from the ring while the FMAs of step ii issue, and the scratch store is a predicated
@@ -141,6 +162,7 @@ __device__ __forceinline__ void fir2_run(const Fir2Params &prm, const uint8_t *w
     for (int i0 = 0; i0 < n_steps; i0 += U) {
 #pragma unroll
         for (int ii = 0; ii < U; ++ii) {
+            if (ii % 8 == 0) sink.before_steps(i0 + ii);
             const uint32_t P0a = nxt[0], P0b = nxt[1], P1a = nxt[2], P1b = nxt[3];
             if ((ii + 1) % kFirBatch == 0) {
                 // the batch that holds step ii + 1 has landed; every lane holds the words of step ii, so the batch
@@ -173,13 +195,12 @@ __device__ __forceinline__ void fir2_run(const Fir2Params &prm, const uint8_t *w
                 cur.w = lagc[1] ? prev.w : now.w;
                 prev = now;
             }
-            asm volatile("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %5, %6;\n\t@p st.global.v4.f32 [%0], {%1, %2, %3, %4};\n\t}"
-                         ::"l"(gp), "f"(cur.x), "f"(cur.y), "f"(cur.z), "f"(cur.w), "r"((unsigned)sp), "r"((unsigned)n_out) : "memory");
-            gp += g_stride;
-            ++sp;
+            sink.store(cur);
+            if (ii % 8 == 7) sink.after_steps(i0 + ii);
         }
     }
     cp_async_wait<0>();
+    sink.end_run();
 }
 
 template <int T>
@@ -208,10 +229,11 @@ __global__ void __launch_bounds__(kFir2Threads, 4) fir2_kernel(const Fir2Params 
         float *grow0 = prm.g + ((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * (int64_t)N * 2;
         const int cr = (int)((int64_t)c & (int64_t)(N - 1));
         const bool mixed = (2 * i_pt + cr < N) && (2 * i_pt + 1 + cr >= N);
+        Fir2ScratchSink sink{grow0 + 4 * i_pt, (size_t)N * 2, 0, 0};
         if (__any_sync(0xffffffffu, mixed))
-            fir2_run<T, true>(prm, wsrc, ring_s, (int64_t)c, m, (int)(run_end - m), i_pt, grow0);
+            fir2_run<T, true>(prm, wsrc, ring_s, (int64_t)c, m, (int)(run_end - m), i_pt, sink);
         else
-            fir2_run<T, false>(prm, wsrc, ring_s, (int64_t)c, m, (int)(run_end - m), i_pt, grow0);
+            fir2_run<T, false>(prm, wsrc, ring_s, (int64_t)c, m, (int)(run_end - m), i_pt, sink);
         m = run_end;
     }
 }

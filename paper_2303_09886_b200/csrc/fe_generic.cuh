@@ -37,7 +37,7 @@ struct GenParams {
 };
 
 // debug: window samples [A][P][S][N*T] int16
-__global__ void gen_unpack_kernel(const GenParams p, int16_t *out)
+static __global__ void gen_unpack_kernel(const GenParams p, int16_t *out)
 {
     const int64_t NT = (int64_t)p.N * p.T;
     const int64_t total = (int64_t)p.A * p.P * p.n_spectra * NT;
@@ -52,7 +52,7 @@ __global__ void gen_unpack_kernel(const GenParams p, int16_t *out)
 }
 
 // Eq. (1), natural column order: g [A][P][S][N]
-__global__ void gen_fir_kernel(const GenParams p, float *g)
+static __global__ void gen_fir_kernel(const GenParams p, float *g)
 {
     const int64_t total = (int64_t)p.A * p.P * p.n_spectra * p.N;
     for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
@@ -73,7 +73,7 @@ __global__ void gen_fir_kernel(const GenParams p, float *g)
 
 // N-point DFT of g (natural order, [A][P][S][N]) + rotation + gain (+ quantise): one thread per channel
 template <bool F32OUT>
-__global__ void gen_dft_kernel(const GenParams p, const float *g, int8_t *out, float *out_f32)
+static __global__ void gen_dft_kernel(const GenParams p, const float *g, int8_t *out, float *out_f32)
 {
     const int n = p.N / 2;
     const int64_t total = (int64_t)p.A * p.P * p.n_spectra * n;
@@ -115,7 +115,7 @@ __global__ void gen_dft_kernel(const GenParams p, const float *g, int8_t *out, f
 
 // debug: undo the rotation and the quad permutation of the tiled FIR's scratch rows:
 // g_out [A][P][S][N] (natural) from g' rows ((a*cap + m)*P + p)
-__global__ void unrotate_kernel(const float *gp, float *g_out, const int32_t *coarse, int64_t n_coarse,
+static __global__ void unrotate_kernel(const float *gp, float *g_out, const int32_t *coarse, int64_t n_coarse,
                                 int64_t n_spectra, int64_t cap, int N, int P, int A)
 {
     const int64_t total = (int64_t)A * P * n_spectra * N;
@@ -139,7 +139,7 @@ __global__ void unrotate_kernel(const float *gp, float *g_out, const int32_t *co
 // (one word = the P (re, im) byte pairs of a channel), heaps is [A][ceil(S/256)][n][256] words; spectra past S in
 // the last heap are zero.  32 x 32-word tiles through shared memory, both sides coalesced.
 template <typename Word>
-__global__ void heaps_transpose_kernel(const Word *__restrict__ rec, Word *__restrict__ heaps, int64_t S, int n)
+static __global__ void heaps_transpose_kernel(const Word *__restrict__ rec, Word *__restrict__ heaps, int64_t S, int n)
 {
     __shared__ Word tile[32][33];
     const int64_t n_heaps = (S + 255) / 256;

@@ -23,8 +23,9 @@
 #include "fe_fir2.cuh"
 #include "fe_fir2b.cuh"
 #include "fe_fir3.cuh"
-#include "fe_fused.cuh"
 #include "fe_generic.cuh"
+#include "fe_pipe.cuh"
+#include "fe_plans.cuh"
 
 using namespace fe;
 
@@ -52,15 +53,22 @@ struct fengine {
     // scratch
     float *d_scratch = nullptr;
     size_t scratch_floats = 0;
-    // fused kernel (fe_fused.cuh): L2-resident ring of scratch slots and its control words
+    // pipelined kernel (fe_pipe.cuh): L2-resident ring of rows and its control words
     float *d_ring = nullptr;
     size_t ring_floats = 0;
     unsigned int *d_ctl = nullptr;
     size_t ctl_words = 0;
-    bool allow_fused = false;       // option "fused" (off by default: see DESIGN.md section 6)
-    int ring_slots = 8;             // option "ring_slots" (D)
-    int lag = 5;                    // option "lag" (phases between a unit's FIR and FFT tasks)
-    int fused_ctas_per_sm = 0;      // option "fused_ctas_per_sm" (0 = occupancy)
+    bool allow_fused = true;        // option "fused": the pipelined kernel is the default where it applies
+    int ring_rows = 32;             // option "ring_rows" (D: rows per track, a power of two >= 16)
+    int opt_fir_warps = 0;          // option "fir_warps" (FIR warps per CTA, 0 = as many as the block allows)
+    int opt_tracks = 0;             // option "tracks" (J, 0 = as many as the FIR warps serve)
+    int opt_segments = 0;           // option "segments" (K per antenna, 0 = chosen per call)
+    int opt_pipe_ctas = 0;          // option "pipe_ctas" (grid, 0 = one CTA per SM)
+    unsigned long long *d_stats = nullptr;   // option "pipe_stats": per-CTA clock counters of the pipelined kernel
+    bool pipe_attr[2] = {};        // kernel variants whose shared-memory attribute is set on this handle's device
+    bool fft_attr[4] = {};          // same for the FFT kernels of the two-kernel path (one plan per handle)
+    bool reserved = false;          // fengine_reserve was called: process never allocates afterwards
+    int device = 0;
     int n_sms = 0;
     // streaming (fengine_stream_*): user coarse delays, row offset folded into the device table, window buffers
     std::vector<int32_t> h_coarse;
@@ -118,19 +126,6 @@ bool all_finite(const float *p, size_t count)
     return true;
 }
 
-// ---- plan list of the tiled FFT: <n, passes, R1, R2, R3, R4, threads per pol-FFT> ----
-using Plan1024 = FftPlan<1024, 3, 8, 8, 16, 1, 64>;
-using Plan2048 = FftPlan<2048, 3, 8, 16, 16, 1, 64>;
-using Plan4096 = FftPlan<4096, 3, 16, 16, 16, 1, 128>;
-using Plan8192 = FftPlan<8192, 4, 8, 8, 8, 16, 256>;
-using Plan16384 = FftPlan<16384, 4, 16, 16, 8, 8, 512>;
-using Plan32768 = FftPlan<32768, 4, 32, 16, 8, 8, 512, 2>;     // two sweeps of 16384 points (fe_fft.cuh)
-
-using Plan2_1024 = Fft2Plan<1024, 8, 8, 128>;
-using Plan2_2048 = Fft2Plan<2048, 8, 16, 128>;
-using Plan2_4096 = Fft2Plan<4096, 16, 16, 256>;
-using Plan2_8192 = Fft2Plan<8192, 16, 16, 256, 2>;    // two sweeps of 4096 points (fe_fft2.cuh)
-
 bool tiled_n(int n) { return n >= 1024 && n <= 32768; }
 bool packed_n(int n) { return n == 1024 || n == 2048 || n == 4096 || n == 8192; }
 bool use_packed(const fengine *fe) { return fe->tiled && fe->packed_ok && fe->pols_equal && fe->allow_packed; }
@@ -166,7 +161,7 @@ template <class Plan, bool F32OUT>
 int launch_fft2(fengine *fe, const Fft2Params &prm, int64_t chunk_len, cudaStream_t stream)
 {
     const size_t smem = fft2_smem_bytes<Plan>();
-    static bool attr_set = false;
+    bool &attr_set = fe->fft_attr[F32OUT ? 1 : 0];      // per handle (= per device), not per process
     if (!attr_set) {
         FE_CUDA(fe, cudaFuncSetAttribute(fft2_kernel<Plan, F32OUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
@@ -198,82 +193,91 @@ bool use_tiled(const fengine *fe)
 }
 bool use_fused(const fengine *fe)
 {
-    return use_packed(fe) && fe->allow_fused && fe->bits == 10 && fe->n <= 4096 && (fe->T == 4 || fe->T == 8 || fe->T == 16);
+    return use_packed(fe) && fe->allow_fused && fe->bits == 10 && (fe->T == 2 || fe->T == 4 || fe->T == 8 || fe->T == 16);
 }
 
-template <int T, class Plan, bool F32OUT>
-int launch_fused(fengine *fe, const FusedParams &prm, cudaStream_t stream)
+// ---- pipelined kernel: work decomposition of a call (fe_pipe.cuh) ----
+struct PipePlan {
+    int FW, J, K, Sseg, D, GP, grid;
+    unsigned int total;
+    size_t ring_floats, ctl_words;
+};
+
+int gcd_int(int a, int b) { return b ? gcd_int(b, a % b) : a; }
+
+PipePlan pipe_plan(const fengine *fe, int64_t S)
 {
-    const size_t smem = fft2_smem_bytes<Plan>();
-    static int ctas_per_sm = 0;
-    if (!ctas_per_sm) {
-        FE_CUDA(fe, cudaFuncSetAttribute(fused2_kernel<T, Plan, F32OUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        FE_CUDA(fe, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, fused2_kernel<T, Plan, F32OUT>, Plan::tpf, smem));
-        if (ctas_per_sm < 1) ctas_per_sm = 1;
+    PipePlan pl{};
+    const int tpf = pipe_team_threads(fe->n);
+    const int fw_max = (kPipeMaxThreads - tpf - 64) / 32;                 // team + loader + flow + FIR warps
+    pl.FW = fe->opt_fir_warps > 0 ? std::min(fe->opt_fir_warps, fw_max) : fw_max;
+    pl.grid = fe->opt_pipe_ctas > 0 ? std::min(fe->opt_pipe_ctas, fe->n_sms) : fe->n_sms;
+    const int wpj = fe->n / 32;
+    while (pl.grid * pl.FW < wpj && pl.FW < fw_max) ++pl.FW;          // at least one track must fit
+    int J = std::max(1, pl.grid * pl.FW / wpj);
+    if (fe->opt_tracks > 0) J = std::min(J, fe->opt_tracks);
+    // segments per antenna: A * K a multiple of J so that every track runs the same number of jobs, as long as a
+    // segment stays long against its T - 1 warm-up rows
+    int K = fe->opt_segments > 0 ? fe->opt_segments : J / gcd_int(fe->A, J);
+    const int64_t min_rows = 8 * (int64_t)fe->T;
+    while (K > 1 && (S + K - 1) / K < min_rows) --K;
+    K = (int)std::max<int64_t>(1, std::min<int64_t>(K, S));
+    pl.K = K;
+    pl.Sseg = (int)((S + K - 1) / K);
+    pl.K = (int)((S + pl.Sseg - 1) / pl.Sseg);                         // drop empty trailing segments
+    const int n_jobs = fe->A * pl.K;
+    pl.J = std::min(J, n_jobs);
+    int D = 16;
+    while (D < fe->ring_rows) D *= 2;
+    pl.D = D;
+    // groups per track: track t runs jobs t, t + J, ...; segment k has ceil(len_k / G) groups
+    int gp = 0;
+    for (int t = 0; t < pl.J; ++t) {
+        int g = 0;
+        for (int j = t; j < n_jobs; j += pl.J) {
+            const int k = j / fe->A;
+            const int64_t len = std::min<int64_t>(pl.Sseg, S - (int64_t)k * pl.Sseg);
+            g += (int)((len + kPipeG - 1) / kPipeG);
+        }
+        gp = std::max(gp, g);
     }
-    const int per_sm = fe->fused_ctas_per_sm > 0 ? fe->fused_ctas_per_sm : ctas_per_sm;
-    // never more CTAs than tasks: a CTA that finds no ticket exits at once, but it still costs a launch slot
-    const int64_t tasks = (int64_t)prm.U * (prm.nb + prm.C);
-    const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>((int64_t)per_sm * fe->n_sms, tasks));
-    fused2_kernel<T, Plan, F32OUT><<<grid, Plan::tpf, smem, stream>>>(prm);
-    return FENGINE_OK;
+    pl.GP = gp;
+    pl.total = (unsigned int)gp * (unsigned int)(pl.J * kPipeG);
+    pl.ring_floats = (size_t)pl.J * pl.D * fe->N * 2;
+    pl.ctl_words = kPipeCtlHeader + 2 * (size_t)pl.J * gp;
+    return pl;
 }
 
-template <int T, bool F32OUT>
-int launch_fused_n(fengine *fe, const FusedParams &prm, cudaStream_t stream)
+// ring and control words of the pipelined kernel for a call of S spectra
+int ensure_pipe(fengine *fe, const PipePlan &pl)
 {
-    switch (fe->n) {
-    case 1024: return launch_fused<T, Plan2_1024, F32OUT>(fe, prm, stream);
-    case 2048: return launch_fused<T, Plan2_2048, F32OUT>(fe, prm, stream);
-    case 4096: return launch_fused<T, Plan2_4096, F32OUT>(fe, prm, stream);
-    }
-    return fail(fe, FENGINE_ERR_INVALID_ARG, "no fused plan for n=%d", fe->n);
-}
-
-template <bool F32OUT>
-int launch_fused_T(fengine *fe, const FusedParams &prm, cudaStream_t stream)
-{
-    switch (fe->T) {
-    case 4: return launch_fused_n<4, F32OUT>(fe, prm, stream);
-    case 8: return launch_fused_n<8, F32OUT>(fe, prm, stream);
-    case 16: return launch_fused_n<16, F32OUT>(fe, prm, stream);
-    }
-    return fail(fe, FENGINE_ERR_INVALID_ARG, "no fused kernel for T=%d", fe->T);
-}
-
-int tpf_of(int n) { return n == 4096 ? Plan2_4096::tpf : n == 2048 ? Plan2_2048::tpf : Plan2_1024::tpf; }
-
-// ring and control words of the fused kernel for a call of S spectra
-int ensure_fused(fengine *fe, int64_t S, int C, int D)
-{
-    const size_t floats = (size_t)D * C * fe->N * 2;
-    if (floats > fe->ring_floats) {
+    if (pl.ring_floats > fe->ring_floats) {
+        if (fe->reserved) return fail(fe, FENGINE_ERR_STATE, "call needs a larger ring than fengine_reserve sized");
         if (fe->d_ring) {
             FE_CUDA(fe, cudaDeviceSynchronize());
             cudaFree(fe->d_ring);
             fe->d_ring = nullptr;
             fe->ring_floats = 0;
         }
-        if (cudaMalloc(&fe->d_ring, floats * sizeof(float)) != cudaSuccess) {
+        if (cudaMalloc(&fe->d_ring, pl.ring_floats * sizeof(float)) != cudaSuccess) {
             cudaGetLastError();
-            return fail(fe, FENGINE_ERR_ALLOC, "cannot allocate %zu bytes of ring", floats * sizeof(float));
+            return fail(fe, FENGINE_ERR_ALLOC, "cannot allocate %zu bytes of ring", pl.ring_floats * sizeof(float));
         }
-        fe->ring_floats = floats;
+        fe->ring_floats = pl.ring_floats;
     }
-    const size_t U = (size_t)((S + C - 1) / C) * fe->A;
-    const size_t words = 4 + 2 * U;
-    if (words > fe->ctl_words) {
+    if (pl.ctl_words > fe->ctl_words) {
+        if (fe->reserved) return fail(fe, FENGINE_ERR_STATE, "call needs more control words than fengine_reserve sized");
         if (fe->d_ctl) {
             FE_CUDA(fe, cudaDeviceSynchronize());
             cudaFree(fe->d_ctl);
             fe->d_ctl = nullptr;
             fe->ctl_words = 0;
         }
-        if (cudaMalloc(&fe->d_ctl, words * sizeof(unsigned int)) != cudaSuccess) {
+        if (cudaMalloc(&fe->d_ctl, pl.ctl_words * sizeof(unsigned int)) != cudaSuccess) {
             cudaGetLastError();
-            return fail(fe, FENGINE_ERR_ALLOC, "cannot allocate the control words of the fused kernel");
+            return fail(fe, FENGINE_ERR_ALLOC, "cannot allocate the control words of the pipelined kernel");
         }
-        fe->ctl_words = words;
+        fe->ctl_words = pl.ctl_words;
     }
     return FENGINE_OK;
 }
@@ -313,7 +317,7 @@ int launch_fft(fengine *fe, const FftParams &prm, int64_t chunk_len, cudaStream_
 {
     const size_t smem = fft_smem_bytes<Plan>(fe->P);
     const size_t smem_max = fft_smem_bytes<Plan>(2);
-    static bool attr_set = false;
+    bool &attr_set = fe->fft_attr[F32OUT ? 3 : 2];
     if (!attr_set) {
         FE_CUDA(fe, cudaFuncSetAttribute(fft_kernel<Plan, F32OUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max));
         FE_CUDA(fe, cudaFuncSetAttribute(fft_kernel<Plan, F32OUT>, cudaFuncAttributePreferredSharedMemoryCarveout,
@@ -356,6 +360,7 @@ int launch_fir(fengine *fe, const FirParams &prm, int64_t chunk_len, cudaStream_
 int ensure_scratch(fengine *fe, size_t floats)
 {
     if (floats <= fe->scratch_floats) return FENGINE_OK;
+    if (fe->reserved) return fail(fe, FENGINE_ERR_STATE, "call needs %zu bytes of scratch, more than fengine_reserve sized", floats * sizeof(float));
     if (fe->d_scratch) {
         FE_CUDA(fe, cudaDeviceSynchronize());
         cudaFree(fe->d_scratch);
@@ -404,7 +409,7 @@ GenParams gen_params(const fengine *fe, const void *in, int64_t S)
     return g;
 }
 
-unsigned gen_grid(int64_t total) { return (unsigned)std::min<int64_t>((total + 255) / 256, 148 * 16); }
+unsigned gen_grid(const fengine *fe, int64_t total) { return (unsigned)std::min<int64_t>((total + 255) / 256, (int64_t)fe->n_sms * 16); }
 
 int check_call(fengine *fe, const void *in, const void *out, int64_t S)
 {
@@ -433,19 +438,19 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
     if (m_hi < 0) m_hi = S;
     if (m_lo == 0) fe->last_launches = 0;
     if (S == 0 || m_hi <= m_lo) return FENGINE_OK;
-    if ((use_fused(fe) || !use_tiled(fe)) && (m_lo != 0 || m_hi != S))
-        return fail(fe, FENGINE_ERR_STATE, "sub-range processing needs the tiled two-kernel path");
+    if (!use_tiled(fe) && (m_lo != 0 || m_hi != S))
+        return fail(fe, FENGINE_ERR_STATE, "sub-range processing needs the tiled kernels");
     const int streams = fe->A * fe->P;
 
     if (!use_tiled(fe)) {
         int rc = ensure_scratch(fe, (size_t)streams * S * fe->N);
         if (rc) return rc;
         const GenParams gp = gen_params(fe, in, S);
-        gen_fir_kernel<<<gen_grid((int64_t)streams * S * fe->N), 256, 0, stream>>>(gp, fe->d_scratch);
+        gen_fir_kernel<<<gen_grid(fe, (int64_t)streams * S * fe->N), 256, 0, stream>>>(gp, fe->d_scratch);
         if (out_f32)
-            gen_dft_kernel<true><<<gen_grid((int64_t)streams * S * fe->n), 256, 0, stream>>>(gp, fe->d_scratch, nullptr, out_f32);
+            gen_dft_kernel<true><<<gen_grid(fe, (int64_t)streams * S * fe->n), 256, 0, stream>>>(gp, fe->d_scratch, nullptr, out_f32);
         else
-            gen_dft_kernel<false><<<gen_grid((int64_t)streams * S * fe->n), 256, 0, stream>>>(gp, fe->d_scratch, out, nullptr);
+            gen_dft_kernel<false><<<gen_grid(fe, (int64_t)streams * S * fe->n), 256, 0, stream>>>(gp, fe->d_scratch, out, nullptr);
         fe->last_launches = 2;
         FE_CUDA(fe, cudaGetLastError());
         return FENGINE_OK;
@@ -539,24 +544,29 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
     }
 
     if (fused) {
-        const int C = (int)std::min<int64_t>(fe->fir_rows > 0 ? fe->fir_rows : 64, S);
-        const int LAG = fe->lag, D = std::max(fe->ring_slots, LAG + 2);
-        rc = ensure_fused(fe, S, C, D);
+        const int64_t Sr = m_hi - m_lo;
+        const PipePlan pl = pipe_plan(fe, Sr);
+        rc = ensure_pipe(fe, pl);
         if (rc) return rc;
-        FusedParams up{};
+        PipeParams up{};
         up.fir = fp2;
         up.fft = xp2;
-        up.fir.m_begin = up.fft.m_begin = 0;
-        up.fir.m_end = up.fft.m_end = S;
+        up.fir.m_begin = up.fft.m_begin = m_lo;
+        up.fir.m_end = up.fft.m_end = m_hi;
         up.ring = fe->d_ring;
         up.ctl = fe->d_ctl;
-        up.S = S;
+        up.m_lo = m_lo;
+        up.S = Sr;
         up.A = fe->A;
-        up.C = C;
-        up.D = D;
-        up.LAG = LAG;
-        up.U = (int)((S + C - 1) / C) * fe->A;
-        up.nb = fe->n / tpf_of(fe->n);
+        up.K = pl.K;
+        up.Sseg = pl.Sseg;
+        up.J = pl.J;
+        up.wpj = fe->n / 32;
+        up.D = pl.D;
+        up.GP = pl.GP;
+        up.fir_warps = pl.FW;
+        up.total_tickets = pl.total;
+        up.stats = fe->d_stats;
         cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
         if (fe->profile) {
             for (auto &e : ev) {
@@ -569,14 +579,15 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
                 fe->ev_used.push_back(e);
             }
             FE_CUDA(fe, cudaEventRecord(ev[0], stream));
-            FE_CUDA(fe, cudaEventRecord(ev[1], stream));    // no separate FIR launch: the whole step is the fused kernel
+            FE_CUDA(fe, cudaEventRecord(ev[1], stream));    // no separate FIR launch: the whole step is one kernel
         }
-        FE_CUDA(fe, cudaMemsetAsync(fe->d_ctl, 0, sizeof(unsigned int) * (4 + 2 * (size_t)up.U), stream));
-        rc = out_f32 ? launch_fused_T<true>(fe, up, stream) : launch_fused_T<false>(fe, up, stream);
-        if (rc) return rc;
+        FE_CUDA(fe, cudaMemsetAsync(fe->d_ctl, 0, sizeof(unsigned int) * pl.ctl_words, stream));
+        bool &attr_set = fe->pipe_attr[out_f32 ? 1 : 0];    // (n, T) are fixed per handle; reset when "fir_warps" changes
+        cudaError_t ce = pipe_launch(fe->T, fe->n, out_f32 != nullptr, up, pl.grid, !attr_set, stream);
+        attr_set = true;
+        if (ce != cudaSuccess) return fail(fe, FENGINE_ERR_CUDA, "pipelined kernel launch failed: %s", cudaGetErrorString(ce));
         if (fe->profile) FE_CUDA(fe, cudaEventRecord(ev[2], stream));
         fe->last_launches += 1;
-        FE_CUDA(fe, cudaGetLastError());
         return FENGINE_OK;
     }
 
@@ -712,6 +723,7 @@ void fengine_destroy(fengine_t *fe)
     cudaFree(fe->d_scratch);
     cudaFree(fe->d_ring);
     cudaFree(fe->d_ctl);
+    cudaFree(fe->d_stats);
     cudaFree(fe->d_win[0]);
     cudaFree(fe->d_win[1]);
     cudaFree(fe->d_rec);
@@ -816,6 +828,26 @@ int fengine_process(fengine_t *fe, const void *in, void *out, int64_t n_spectra,
     if (rc) return rc;
     if (fe->stream_off != 0) return fail(fe, FENGINE_ERR_STATE, "a stream is open: use fengine_stream_push or fengine_stream_end");
     return process_impl(fe, in, static_cast<int8_t *>(out), nullptr, n_spectra, static_cast<cudaStream_t>(stream));
+}
+
+int fengine_reserve(fengine_t *fe, int64_t max_spectra)
+{
+    if (!fe) return FENGINE_ERR_INVALID_ARG;
+    fe->err.clear();
+    if (max_spectra < 1) return fail(fe, FENGINE_ERR_INVALID_ARG, "max_spectra < 1");
+    fe->reserved = false;                                   // this call may allocate; later process calls may not
+    int rc = FENGINE_OK;
+    if (use_tiled(fe) && use_fused(fe)) {
+        // the ring does not depend on S; the counters grow with it (every smaller call needs no more of either)
+        rc = ensure_pipe(fe, pipe_plan(fe, max_spectra));
+    } else {
+        const int64_t chunk = fe->chunk_spectra > 0 ? std::min<int64_t>(fe->chunk_spectra, max_spectra) : max_spectra;
+        rc = ensure_scratch(fe, (size_t)fe->A * fe->P * (size_t)chunk * fe->N);
+    }
+    if (rc) return rc;
+    FE_CUDA(fe, cudaDeviceSynchronize());
+    fe->reserved = true;
+    return FENGINE_OK;
 }
 
 int fengine_process_heaps(fengine_t *fe, const void *in, void *heaps_out, int64_t n_spectra, void *stream)
@@ -981,7 +1013,7 @@ int fengine_process_host(fengine_t *fe, const void *in_host, void *out_host, int
     // host_chunks pieces of spectra; the input rows a piece needs go up on one stream, the piece is processed on a
     // second and its output records come down on a third, so that PCIe runs in both directions under the kernels.
     const int K = fe->host_chunks;
-    if (use_tiled(fe) && !use_fused(fe) && K > 1 && n_spectra >= 4 * (int64_t)K) {
+    if (use_tiled(fe) && K > 1 && n_spectra >= 4 * (int64_t)K) {
         const int64_t S = n_spectra, rows_in = S + fe->T - 1;
         const size_t row_bytes = (size_t)fe->N / 8 * fe->bits, stream_bytes = row_bytes * rows_in;
         const int n_streams = fe->A * fe->P;
@@ -1050,7 +1082,7 @@ int fengine_debug_unpack(fengine_t *fe, const void *in, int16_t *samples_out, in
     if (rc || n_spectra == 0) return rc;
     const GenParams gp = gen_params(fe, in, n_spectra);
     const int64_t total = (int64_t)fe->A * fe->P * n_spectra * fe->N * fe->T;
-    gen_unpack_kernel<<<gen_grid(total), 256, 0, static_cast<cudaStream_t>(stream)>>>(gp, samples_out);
+    gen_unpack_kernel<<<gen_grid(fe, total), 256, 0, static_cast<cudaStream_t>(stream)>>>(gp, samples_out);
     FE_CUDA(fe, cudaGetLastError());
     return FENGINE_OK;
 }
@@ -1062,7 +1094,7 @@ int fengine_debug_fir(fengine_t *fe, const void *in, float *g_out, int64_t n_spe
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const int64_t total = (int64_t)fe->A * fe->P * n_spectra * fe->N;
     if (!use_tiled(fe)) {
-        gen_fir_kernel<<<gen_grid(total), 256, 0, s>>>(gen_params(fe, in, n_spectra), g_out);
+        gen_fir_kernel<<<gen_grid(fe, total), 256, 0, s>>>(gen_params(fe, in, n_spectra), g_out);
     } else if (use_packed(fe)) {
         rc = ensure_scratch(fe, (size_t)total);
         if (rc) return rc;
@@ -1081,7 +1113,7 @@ int fengine_debug_fir(fengine_t *fe, const void *in, float *g_out, int64_t n_spe
         fp.rows_per_tile = fir_rows_for(fe, n_spectra, 2 * kFir2Threads, 2);
         rc = launch_fir2(fe, fp, n_spectra, s);
         if (rc) return rc;
-        unrotate2_kernel<<<gen_grid(total), 256, 0, s>>>(fe->d_scratch, g_out, fe->d_coarse, fe->n_coarse, n_spectra,
+        unrotate2_kernel<<<gen_grid(fe, total), 256, 0, s>>>(fe->d_scratch, g_out, fe->d_coarse, fe->n_coarse, n_spectra,
                                                          n_spectra, fe->N, fe->A);
     } else {
         rc = ensure_scratch(fe, (size_t)total);
@@ -1102,7 +1134,7 @@ int fengine_debug_fir(fengine_t *fe, const void *in, float *g_out, int64_t n_spe
         fp.rows_per_tile = fir_rows_for(fe, n_spectra, kFirColsPerBlock, 1);
         rc = launch_fir(fe, fp, n_spectra, s);
         if (rc) return rc;
-        unrotate_kernel<<<gen_grid(total), 256, 0, s>>>(fe->d_scratch, g_out, fe->d_coarse, fe->n_coarse, n_spectra,
+        unrotate_kernel<<<gen_grid(fe, total), 256, 0, s>>>(fe->d_scratch, g_out, fe->d_coarse, fe->n_coarse, n_spectra,
                                                         n_spectra, fe->N, fe->P, fe->A);
     }
     FE_CUDA(fe, cudaGetLastError());
@@ -1148,19 +1180,26 @@ int fengine_set_option(fengine_t *fe, const char *key, int64_t value)
         fe->allow_fused = value != 0;
         return FENGINE_OK;
     }
-    if (!strcmp(key, "ring_slots")) {
-        if (value < 2 || value > 1024) return fail(fe, FENGINE_ERR_INVALID_ARG, "ring_slots out of range");
-        fe->ring_slots = (int)value;
+    if (!strcmp(key, "ring_rows")) {
+        if (value < 16 || value > 4096) return fail(fe, FENGINE_ERR_INVALID_ARG, "ring_rows out of range");
+        fe->ring_rows = (int)value;
         return FENGINE_OK;
     }
-    if (!strcmp(key, "lag")) {
-        if (value < 1 || value > 1022) return fail(fe, FENGINE_ERR_INVALID_ARG, "lag out of range");
-        fe->lag = (int)value;
+    if (!strcmp(key, "fir_warps") || !strcmp(key, "tracks") || !strcmp(key, "segments") || !strcmp(key, "pipe_ctas")) {
+        if (value < 0 || value > 65536) return fail(fe, FENGINE_ERR_INVALID_ARG, "%s out of range", key);
+        (key[0] == 'f' ? fe->opt_fir_warps : key[0] == 't' ? fe->opt_tracks : key[0] == 's' ? fe->opt_segments : fe->opt_pipe_ctas) = (int)value;
+        fe->pipe_attr[0] = fe->pipe_attr[1] = false;        // the shared-memory size follows fir_warps
         return FENGINE_OK;
     }
-    if (!strcmp(key, "fused_ctas_per_sm")) {
-        if (value < 0 || value > 32) return fail(fe, FENGINE_ERR_INVALID_ARG, "fused_ctas_per_sm out of range");
-        fe->fused_ctas_per_sm = (int)value;
+    if (!strcmp(key, "pipe_stats")) {                       // 1: allocate and zero the counters; 0: off
+        FE_CUDA(fe, cudaDeviceSynchronize());
+        cudaFree(fe->d_stats);
+        fe->d_stats = nullptr;
+        if (value) {
+            const size_t bytes = sizeof(unsigned long long) * kStCount * (size_t)fe->n_sms;
+            FE_CUDA(fe, cudaMalloc(&fe->d_stats, bytes));
+            FE_CUDA(fe, cudaMemset(fe->d_stats, 0, bytes));
+        }
         return FENGINE_OK;
     }
     if (!strcmp(key, "force_generic")) {
@@ -1195,5 +1234,17 @@ int fengine_profile_read(fengine_t *fe, double *fir_ms, double *fft_ms, int64_t 
 }
 
 int64_t fengine_last_launch_count(const fengine_t *fe) { return fe ? fe->last_launches : 0; }
+
+int fengine_debug_pipe_stats(fengine_t *fe, uint64_t *out, int64_t max_words)
+{
+    if (!fe || !out) return FENGINE_ERR_INVALID_ARG;
+    fe->err.clear();
+    if (!fe->d_stats) return fail(fe, FENGINE_ERR_STATE, "option pipe_stats is off");
+    const int64_t words = std::min<int64_t>(max_words, (int64_t)kStCount * fe->n_sms);
+    FE_CUDA(fe, cudaDeviceSynchronize());
+    FE_CUDA(fe, cudaMemcpy(out, fe->d_stats, sizeof(uint64_t) * (size_t)words, cudaMemcpyDeviceToHost));
+    FE_CUDA(fe, cudaMemset(fe->d_stats, 0, sizeof(unsigned long long) * kStCount * (size_t)fe->n_sms));
+    return FENGINE_OK;
+}
 
 }  // extern "C"

@@ -379,14 +379,18 @@ def test_chunking_and_tile_size_do_not_change_results(torch, fb):
 
 
 @pytest.mark.parametrize("n,T,S,A,per_spectrum,opts", [
-    (1024, 16, 128, 1, False, dict(fir_rows=64)),                       # config-1 shape, two units
-    (1024, 8, 37, 3, False, dict(fir_rows=8, ring_slots=3, lag=1)),     # ragged last unit, smallest ring: slot reuse waits
-    (2048, 4, 70, 2, True, dict(fir_rows=16, ring_slots=4, lag=2)),     # per-spectrum delays (equal in both pols)
-    (4096, 16, 150, 2, False, dict(fir_rows=64, ring_slots=8, lag=5)),
-    (4096, 16, 3, 1, False, dict(fir_rows=64)),                         # fewer rows than one unit
+    (1024, 16, 128, 1, False, dict()),                                  # config-1 shape
+    (1024, 8, 37, 3, False, dict(ring_rows=16, segments=2)),            # smallest ring: slot reuse waits; ragged segments
+    (2048, 4, 70, 2, True, dict(ring_rows=16)),                         # per-spectrum delays (equal in both pols)
+    (4096, 16, 150, 2, False, dict()),
+    (4096, 16, 333, 1, False, dict(segments=5, tracks=3, ring_rows=16)),  # more jobs than tracks: tracks run job after job
+    (4096, 16, 3, 1, False, dict()),                                    # fewer rows than one group
+    (8192, 16, 90, 2, False, dict()),                                   # two-sweep FFT out of one landing buffer
+    (8192, 8, 45, 1, True, dict(ring_rows=16, segments=3)),
+    (4096, 2, 40, 1, False, dict(fir_warps=3)),                         # fewer FIR warps per CTA than the block allows
 ])
 def test_fused_kernel_matches_oracle_and_two_kernel_path(torch, fb, n, T, S, A, per_spectrum, opts):
-    """The persistent fused kernel (fe_fused.cuh: L2-resident ring, ticket order, release/acquire counters)."""
+    """The pipelined kernel (fe_pipe.cuh: persistent FIR warps -> L2-resident ring -> bulk copies -> FFT team)."""
     w = si.custom_workload(A=A, n=n, T=T, S=S, P=2, seed=31, per_spectrum=per_spectrum, coarse_range=(0, 3 * n))
     w.coarse[:, 1] = w.coarse[:, 0]                  # the pol-packed kernels need equal coarse delays in both pols
     ref = oracle_run(w)
@@ -398,7 +402,7 @@ def test_fused_kernel_matches_oracle_and_two_kernel_path(torch, fb, n, T, S, A, 
 
 def test_fused_kernel_repeated_calls_are_deterministic(torch, fb):
     w = si.make_workload(2, n_spectra=200, n_antennas=2)
-    fe = make_engine(fb, w, fused=1, fir_rows=32, ring_slots=5, lag=3)
+    fe = make_engine(fb, w, fused=1, ring_rows=16)
     first = gpu_run(torch, fe, w, want=("int8",))["out"]
     for _ in range(3):
         np.testing.assert_array_equal(first, gpu_run(torch, fe, w, want=("int8",))["out"])
