@@ -58,7 +58,7 @@ struct fengine {
     size_t ring_floats = 0;
     unsigned int *d_ctl = nullptr;
     size_t ctl_words = 0;
-    bool allow_fused = true;        // option "fused": the pipelined kernel is the default where it applies
+    bool allow_fused = false;       // option "fused": the pipelined kernel (fe_pipe.cuh), slower than the two-kernel path today
     int ring_rows = 32;             // option "ring_rows" (D: rows per track, a power of two >= 16)
     int opt_fir_warps = 0;          // option "fir_warps" (FIR warps per CTA, 0 = as many as the block allows)
     int opt_tracks = 0;             // option "tracks" (J, 0 = as many as the FIR warps serve)
