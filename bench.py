@@ -32,6 +32,16 @@ UNIT = "Gsample/s"
 ALG_BYTES_PER_DUALPOL_SAMPLE = 4.5     # 1.25 B in + 1 B out per real sample, x2 pols
 
 
+def csrc_hash() -> str:
+    """sha256 over the kernel sources (sorted by name): ties profiles/roofline_traffic.csv to the code it measured."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted((ROOT / "paper_2303_09886_b200" / "csrc").glob("*.cu*")):
+        h.update(f.name.encode())
+        h.update(f.read_bytes())
+    return h.hexdigest()
+
+
 def measured_peaks():
     f = ROOT / "MEASURED_PEAKS.json"
     if f.exists():
@@ -139,7 +149,7 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2)
@@ -152,7 +162,11 @@ def main():
     ap.add_argument("--opt", action="append", default=[], help="library option key=value (fengine_set_option), repeatable")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--csrc-hash", action="store_true", help="print the kernel-source hash that profiles/roofline_traffic.csv is stamped with")
     args = ap.parse_args()
+    if args.csrc_hash:
+        print(csrc_hash())
+        return 0
     if args.impl == "reference":
         return run_reference(args)
 
@@ -210,14 +224,21 @@ def main():
     barrier()
     sampler = ClockSampler(local_rank)
     time.sleep(0.15)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    # one event per step boundary (recorded on the stream the kernels are launched on): the bracketing pair gives
+    # the contract's K-step time, the inner ones the per-step distribution (median and spread)
+    marks = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     barrier()
-    e0.record()
+    marks[0].record()
     for i in range(args.steps):
         step(i)
-    e1.record()
+        marks[i + 1].record()
     barrier()
-    ms_total = e0.elapsed_time(e1)
+    ms_total = marks[0].elapsed_time(marks[-1])
+    per_step = sorted(marks[i].elapsed_time(marks[i + 1]) for i in range(args.steps))
+    def pct(q):
+        return per_step[min(len(per_step) - 1, int(q * len(per_step)))]
+    step_stats = {"median": statistics.median(per_step), "p10": pct(0.10), "p90": pct(0.90), "min": per_step[0],
+                  "max": per_step[-1], "n": len(per_step)}
     launches = fe.last_launch_count() * args.steps
     # keep the GPU busy a little longer so the clock sampler sees enough loaded samples
     t_end = time.time() + 0.6
@@ -236,14 +257,15 @@ def main():
 
     # ---- per-kernel durations (CUDA events recorded by the library on the launching stream) ----
     fe.set_option("profile", 1)
-    for i in range(args.steps):
+    n_prof = min(args.steps, 50)
+    for i in range(n_prof):
         step(i)
     torch.cuda.synchronize()
     fir_ms, fft_ms, n_fir, n_fft = fe.profile_read()
     fe.set_option("profile", 0)
     peak, peak_src = measured_peaks()
     fir_avg, fft_avg = fir_ms / max(n_fir, 1), fft_ms / max(n_fft, 1)
-    launches_per_step = max(n_fir // max(args.steps, 1), 1)
+    launches_per_step = max(n_fir // max(n_prof, 1), 1)
     dom_name, dom_avg = ("fft_kernel", fft_avg) if fft_avg >= fir_avg else ("fir_kernel", fir_avg)
     alg_bytes_per_unit = 2.0 * (args.sample_bits / 8.0 + 1.0)      # 4.5 at 10 bits (ALG_BYTES_PER_DUALPOL_SAMPLE)
     alg_bytes_launch = alg_bytes_per_unit * units_per_step / launches_per_step
@@ -260,24 +282,40 @@ def main():
     }
     # The path is bound by the plain FP32 pipe before it is bound by HBM:
     # north-star accounting, FIR 2T flop + FFT 5 n log2(n) / N flop per real sample; an FMA is one lane-operation
-    # (2 flop), the FFT's adds and multiplies are one lane-operation each.  Peak = measured packed-FP32 issue rate
-    # (profiles/r1_fp32_rate.txt: 125.5 lane-ops/clk/SM x 148 SMs x 1.965 GHz).
+    # (2 flop), the FFT's adds and multiplies are one lane-operation each.  Peak = the packed-FP32 issue rate the
+    # library measures in this run (fengine_debug_fp32_rate; about 124 lane-ops/clk/SM, profiles/r1_fp32_rate.txt).
     lane_ops_per_real = w.T + 5.0 * w.n * np.log2(w.n) / w.N
-    alu_peak = 125.5 * 148 * 1.965e9
+    alu_peak = fb.fp32_rate()                            # measured now, on this device, at the clocks of the moment
     alu_achieved = lane_ops_per_real * w.P * units_per_step / (ms_per_step * 1e-3)
     roofline["alu"] = {"bound": "alu", "achieved": alu_achieved / 1e12, "peak": alu_peak / 1e12, "unit": "T lane-op/s",
                        "frac": alu_achieved / alu_peak, "lane_ops_per_real_sample": lane_ops_per_real,
+                       "peak_source": "fengine_debug_fp32_rate in this run (packed FFMA2 loop on every SM)",
                        "note": "whole step against the measured FP32 issue rate; the slower of this and the HBM roofline "
                                "is the north star's roofline"}
     roofline["fused"] = bool(n_fir and fir_avg < 0.02 * max(fft_avg, 1e-9))
     if roofline["fused"]:
         roofline["kernel"] = dom_name = "fused_kernel"
-    prof = ROOT / "profiles" / "roofline_traffic.csv"       # ncu dram bytes per launch of the committed capture
+    # DRAM bytes per launch come from a committed `ncu --set full` capture (a number taken under the profiler is never
+    # a bench value, and ncu cannot run inside this timed program).  The CSV names the sha256 of the kernel sources it
+    # was taken from; when the sources have changed since, the figures are withheld (null) instead of going stale.
+    prof = ROOT / "profiles" / "roofline_traffic.csv"
+    roofline["traffic_step"] = None
     if prof.exists():
+        rows, src_hash = {}, None
         for ln in prof.read_text().splitlines():
+            if ln.startswith("# csrc_sha256="):
+                src_hash = ln.split("=", 1)[1].strip()
             parts = ln.split(",")
-            if len(parts) == 2 and parts[0] == dom_name and parts[1].isdigit():
-                roofline["traffic"] = int(parts[1])
+            if len(parts) == 2 and parts[1].isdigit():
+                rows[parts[0]] = int(parts[1])
+        if src_hash == csrc_hash():
+            roofline["traffic"] = rows.get(dom_name)
+            names = ["fused_kernel"] if roofline["fused"] else ["fir_kernel", "fft_kernel"]
+            if all(nm in rows for nm in names):
+                roofline["traffic_step"] = sum(rows[nm] for nm in names)
+            roofline["traffic_source"] = f"profiles/roofline_traffic.csv (ncu capture of these sources, sha256 {src_hash[:12]})"
+        else:
+            roofline["traffic_source"] = "withheld: csrc/ has changed since the committed ncu capture (profiles/roofline_traffic.csv)"
 
     # ---- end to end through fengine_process_host: pinned host buffers, H2D + path + D2H per step ----
     e2e = None
@@ -315,7 +353,7 @@ def main():
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms_per_step, "ms_per_step_stats": step_stats, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": f"config{args.config}: {w.A} antennas x {w.P} pols per GPU, n={w.n}, T={w.T}, "
                                    f"{w.L} samples per pol per step, S={w.S} spectra",

@@ -17,9 +17,14 @@
  * Conventions
  *   - plain C, no torch types; "host" / "device" is stated for every pointer.
  *   - every function returning int returns a FENGINE_* status; nothing is thrown across the ABI.
- *   - a handle is not thread-safe; independent handles are independent.
+ *   - a handle is not thread-safe and is driven from ONE CUDA stream at a time (its scratch and tables are
+ *     shared by all calls): order calls on different streams yourself (events) or use one handle per stream.
+ *     Independent handles are independent.  A handle belongs to the device that was current at create; calls
+ *     made with another current device fail with FENGINE_ERR_STATE.
  *   - setters copy their host arrays before returning (caller keeps ownership) and take effect
- *     for later fengine_process calls.  They synchronise the device (off the hot path).
+ *     for later fengine_process calls.  They rebuild the derived tables and synchronise the device before
+ *     AND after (off the hot path), so a later call on any stream, blocking or not, sees the new values;
+ *     fengine_process itself never launches a table kernel.
  *   - there is no CPU fallback: without a CUDA device every call fails with FENGINE_ERR_CUDA.
  */
 #ifndef FENGINE_H
@@ -180,14 +185,16 @@ int fengine_debug_fir(fengine_t *fe, const void *in, float *g_out, int64_t n_spe
  * L2-resident chunk; 0 = whole call), "fir_rows" (spectra per FIR tile), "profile" (0/1, see below), "force_generic" (0/1: use the simple
  * one-thread-per-output kernels), "pol_packed" (0/1, default 1: allow the kernels that process both pols of an
  * antenna in packed FP32 lanes; they are used when n_pols = 2, n <= 8192 and the two pols of every antenna have
- * equal coarse delays), "fused" (0/1, default 0: run the pol-packed path as ONE persistent kernel whose FIR -> FFT
- * transposition goes through an L2-resident ring of scratch slots instead of a full-size HBM scratch; T = 4, 8, 16),
- * "ring_slots" / "lag" (ring depth D and FIR-to-FFT phase distance of the fused kernel, D >= lag + 2 is enforced),
- * "fused_ctas_per_sm" (0 = occupancy), "host_chunks" (pieces of the fengine_process_host pipeline, 1 = no overlap),
+ * equal coarse delays), "fused" (0/1, default 0: run the pol-packed path as ONE persistent, warp-specialised kernel
+ * whose FIR -> FFT transposition goes through an L2-resident ring of rows instead of a full-size HBM scratch,
+ * fe_pipe.cuh; T = 2, 4, 8, 16; knobs "ring_rows", "fir_warps", "tracks", "segments", "pipe_ctas"), "split" (0/1,
+ * default 0, n = 4096: the first radix-16 stage of the transform runs in the FIR kernel and the rest as independent
+ * 256-point transforms per warp, fe_split.cuh, the arrangement PAPER.md:403-409 proposes), "host_chunks" (pieces of the fengine_process_host pipeline, 1 = no overlap),
  * "sample_bits" (4, 8, 10 (default), 12, 16: width of the packed input samples, same big-endian bit stream, sample u
  * in bits [b u, b u + b); the stream is then L*b/8 bytes.  The paper's bit-depth sweep.  Widths other
  * than 10 run the tiled kernels on the pol-packed path with 16 taps, else the generic kernels).  Returns INVALID_ARG for
- * unknown keys. */
+ * unknown keys, and STATE for the options that change the data layout or the path ("sample_bits", "force_generic",
+ * "pol_packed", "fused", "split") while a stream is open. */
 int fengine_set_option(fengine_t *fe, const char *key, int64_t value);
 
 /*
@@ -206,6 +213,14 @@ int64_t fengine_last_launch_count(const fengine_t *fe);
  * three roles, rows per team; layout in csrc/fe_pipe.cuh).  Copies up to max_words of them to HOST `out`
  * ([n_sms][16] uint64) and zeroes them.  Synchronises the device. */
 int fengine_debug_pipe_stats(fengine_t *fe, uint64_t *out, int64_t max_words);
+
+/* Measurement hook for the "alu" roofline (BASELINE.json north_star: "the FIR+FFT flops at FP32 peak"; the FIR of
+ * Eq. (1), is 2T flops per sample in exactly this instruction form): runs a loop of packed FP32
+ * multiply-adds (FFMA2, the FIR kernels' operand pattern) on every SM of the current device, a few launches timed with
+ * CUDA events on the legacy stream, and writes the sustained rate in lane-operations (one FMA = one lane-operation)
+ * per second to HOST *lane_ops_per_second and the time of one launch in ms to HOST *ms_per_launch (may be NULL).
+ * Needs no handle; synchronises the device. */
+int fengine_debug_fp32_rate(double *lane_ops_per_second, double *ms_per_launch);
 
 #ifdef __cplusplus
 }

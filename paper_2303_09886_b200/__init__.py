@@ -11,4 +11,5 @@ from .binding import (  # noqa: F401
     lib,
     library_path,
     EXPORTED_SYMBOLS,
+    fp32_rate,
 )

@@ -16,7 +16,7 @@ EXPORTED_SYMBOLS = [
     "fengine_set_fine_delays", "fengine_set_gains", "fengine_process", "fengine_process_host",
     "fengine_last_error", "fengine_process_f32", "fengine_debug_unpack", "fengine_debug_fir",
     "fengine_set_option", "fengine_last_launch_count", "fengine_profile_read", "fengine_process_heaps",
-    "fengine_stream_begin", "fengine_stream_push", "fengine_stream_end", "fengine_reserve", "fengine_debug_pipe_stats",
+    "fengine_stream_begin", "fengine_stream_push", "fengine_stream_end", "fengine_reserve", "fengine_debug_pipe_stats", "fengine_debug_fp32_rate",
 ]
 
 STATUS = {0: "OK", 1: "INVALID_ARG", 2: "ALLOC", 3: "CUDA", 4: "STATE"}
@@ -55,6 +55,7 @@ def lib() -> C.CDLL:
         L.fengine_process_host.argtypes = [vp, vp, vp, i64]
         L.fengine_reserve.argtypes = [vp, i64]
         L.fengine_debug_pipe_stats.argtypes = [vp, vp, i64]
+        L.fengine_debug_fp32_rate.argtypes = [vp, vp]
         L.fengine_process_heaps.argtypes = [vp, vp, vp, i64, vp]
         L.fengine_stream_begin.argtypes = [vp, i64, vp]
         L.fengine_stream_push.argtypes = [vp, vp, vp, i64, vp]
@@ -85,6 +86,20 @@ def _dev_ptr(t) -> int:
     return t.data_ptr()
 
 
+def _dev_buf(t, need_bytes: int, what: str, dtypes=None) -> int:
+    """Device pointer of a contiguous CUDA tensor holding at least need_bytes (raw ints pass unchecked)."""
+    if isinstance(t, int):
+        return t
+    if not t.is_cuda or not t.is_contiguous():
+        raise ValueError(f"{what}: expected a contiguous CUDA tensor")
+    if dtypes is not None and str(t.dtype).replace("torch.", "") not in dtypes:
+        raise ValueError(f"{what}: dtype {t.dtype}, expected one of {dtypes}")
+    have = t.numel() * t.element_size()
+    if have < need_bytes:
+        raise ValueError(f"{what}: {have} bytes, the call needs {need_bytes}")
+    return t.data_ptr()
+
+
 def _stream_handle(stream) -> int:
     if stream is None:
         import torch
@@ -92,6 +107,15 @@ def _stream_handle(stream) -> int:
     if isinstance(stream, int):
         return stream
     return stream.cuda_stream
+
+
+def fp32_rate() -> float:
+    """fengine_debug_fp32_rate: sustained packed-FP32 rate of the current device in lane-operations per second."""
+    r, ms = C.c_double(), C.c_double()
+    rc = lib().fengine_debug_fp32_rate(C.byref(r), C.byref(ms))
+    if rc != 0:
+        raise FEngineError(rc, "fengine_debug_fp32_rate failed")
+    return float(r.value)
 
 
 class FEngine:
@@ -156,17 +180,27 @@ class FEngine:
         """fengine_reserve: size every buffer now so that process() never allocates."""
         self._check(self._lib.fengine_reserve(self._h, int(max_spectra)))
 
+    def _in(self, t, n_spectra: int) -> int:
+        return _dev_buf(t, self.input_bytes(max(n_spectra, 0)) if n_spectra > 0 else 0, "input", ("uint8", "int8"))
+
+    def _out(self, t, n_spectra: int, itemsize: int = 1, dtypes=("int8", "uint8")) -> int:
+        need = int(np.prod(self.output_shape(max(n_spectra, 0)))) * itemsize
+        return _dev_buf(t, need, "output", dtypes)
+
     # -- the hot path -----------------------------------------------------------------------------
     def process(self, inp, out, n_spectra: int, stream=None):
         """fengine_process: device tensors (uint8 in, int8 out); asynchronous on `stream`."""
-        self._check(self._lib.fengine_process(self._h, _dev_ptr(inp), _dev_ptr(out), n_spectra, _stream_handle(stream)))
+        self._check(self._lib.fengine_process(self._h, self._in(inp, n_spectra), self._out(out, n_spectra), n_spectra,
+                                              _stream_handle(stream)))
 
     def heaps_shape(self, n_spectra: int):
         return (self.A, (n_spectra + 255) // 256, self.n, 256, self.P, 2)
 
     def process_heaps(self, inp, heaps_out, n_spectra: int, stream=None):
         """fengine_process_heaps: channel-major heaps of 256 spectra (int8, shape heaps_shape(n_spectra))."""
-        self._check(self._lib.fengine_process_heaps(self._h, _dev_ptr(inp), _dev_ptr(heaps_out), n_spectra,
+        need = int(np.prod(self.heaps_shape(max(n_spectra, 0))))
+        self._check(self._lib.fengine_process_heaps(self._h, self._in(inp, n_spectra),
+                                                    _dev_buf(heaps_out, need, "heaps", ("int8", "uint8")), n_spectra,
                                                     _stream_handle(stream)))
 
     def stream_begin(self, max_new_spectra: int) -> int:
@@ -176,30 +210,42 @@ class FEngine:
         return int(d.value)
 
     def stream_push(self, inp_new, out, n_new: int, stream=None):
-        self._check(self._lib.fengine_stream_push(self._h, _dev_ptr(inp_new), _dev_ptr(out), n_new, _stream_handle(stream)))
+        row_bytes = self.N * getattr(self, "sample_bits", 10) // 8
+        need_in = self.A * self.P * max(n_new, 0) * row_bytes                  # the new rows only: the library keeps history
+        self._check(self._lib.fengine_stream_push(self._h, _dev_buf(inp_new, need_in, "input", ("uint8", "int8")),
+                                                  self._out(out, n_new), n_new, _stream_handle(stream)))
 
     def stream_end(self):
         self._check(self._lib.fengine_stream_end(self._h))
 
     def process_f32(self, inp, out_f32, n_spectra: int, stream=None):
-        self._check(self._lib.fengine_process_f32(self._h, _dev_ptr(inp), _dev_ptr(out_f32), n_spectra,
+        self._check(self._lib.fengine_process_f32(self._h, self._in(inp, n_spectra),
+                                                  self._out(out_f32, n_spectra, 4, ("float32",)), n_spectra,
                                                   _stream_handle(stream)))
 
     def process_host(self, inp_host, out_host, n_spectra: int):
         """fengine_process_host: host buffers (numpy or pinned torch tensors); synchronous."""
-        def hp(x):
+        def hp(x, need, what):
             if isinstance(x, np.ndarray):
+                if not x.flags["C_CONTIGUOUS"] or x.nbytes < need:
+                    raise ValueError(f"{what}: expected a C-contiguous array of at least {need} bytes")
                 return x.ctypes.data
+            if x.is_cuda or not x.is_contiguous() or x.numel() * x.element_size() < need:
+                raise ValueError(f"{what}: expected a contiguous host tensor of at least {need} bytes")
             return x.data_ptr()
-        self._check(self._lib.fengine_process_host(self._h, hp(inp_host), hp(out_host), n_spectra))
+        n_out = int(np.prod(self.output_shape(max(n_spectra, 0))))
+        self._check(self._lib.fengine_process_host(self._h, hp(inp_host, self.input_bytes(n_spectra) if n_spectra > 0 else 0, "input"),
+                                                   hp(out_host, n_out, "output"), n_spectra))
 
     def debug_unpack(self, inp, out_i16, n_spectra: int, stream=None):
-        self._check(self._lib.fengine_debug_unpack(self._h, _dev_ptr(inp), _dev_ptr(out_i16), n_spectra,
-                                                   _stream_handle(stream)))
+        need = self.A * self.P * max(n_spectra, 0) * self.N * self.T * 2
+        self._check(self._lib.fengine_debug_unpack(self._h, self._in(inp, n_spectra), _dev_buf(out_i16, need, "samples", ("int16",)),
+                                                   n_spectra, _stream_handle(stream)))
 
     def debug_fir(self, inp, out_f32, n_spectra: int, stream=None):
-        self._check(self._lib.fengine_debug_fir(self._h, _dev_ptr(inp), _dev_ptr(out_f32), n_spectra,
-                                                _stream_handle(stream)))
+        need = self.A * self.P * max(n_spectra, 0) * self.N * 4
+        self._check(self._lib.fengine_debug_fir(self._h, self._in(inp, n_spectra), _dev_buf(out_f32, need, "g", ("float32",)),
+                                                n_spectra, _stream_handle(stream)))
 
     def profile_read(self):
         """(fir_ms, fft_ms, n_fir, n_fft) summed since the last read (option "profile" must be 1)."""

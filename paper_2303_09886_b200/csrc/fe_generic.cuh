@@ -156,4 +156,31 @@ static __global__ void heaps_transpose_kernel(const Word *__restrict__ rec, Word
         dst[(int64_t)(k0 + j) * 256 + s0 + threadIdx.x] = tile[threadIdx.x][j];
 }
 
+
+// Measurement hook (fengine_debug_fp32_rate): the FIR's instruction form, one sample pair against 16 scalar weights
+// into 16 accumulator pairs (FFMA2, the sample operand reused), in a loop that does nothing else.  What it sustains is
+// the denominator of the "alu" roofline of bench.py; the path's butterflies (FADD2 / FMUL2)
+// issue at the same rate, an FFMA2 with three fresh operands at about three quarters of it.
+constexpr int kRateIters = 2048;
+static __global__ void __launch_bounds__(1024, 1) fp32_rate_kernel(float *out, float a0, float b0)
+{
+    float2 acc[16];
+    float w[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        acc[i] = make_float2(threadIdx.x * 1e-3f + i, i * 0.5f);
+        w[i] = b0 + i * 0.01f + threadIdx.x * 1e-7f;
+    }
+    float2 s = make_float2(a0 + threadIdx.x * 1e-6f, a0 - 1.0f);
+    for (int it = 0; it < kRateIters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) acc[i] = __ffma2_rn(s, make_float2(w[i], w[i]), acc[i]);
+        s.x = -s.x;
+    }
+    float r = 0;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) r += acc[i].x + acc[i].y;
+    out[blockIdx.x * blockDim.x + threadIdx.x] = r;
+}
+
 }  // namespace fe

@@ -26,6 +26,7 @@
 #include "fe_generic.cuh"
 #include "fe_pipe.cuh"
 #include "fe_plans.cuh"
+#include "fe_split.cuh"
 
 using namespace fe;
 
@@ -59,6 +60,9 @@ struct fengine {
     unsigned int *d_ctl = nullptr;
     size_t ctl_words = 0;
     bool allow_fused = false;       // option "fused": the pipelined kernel (fe_pipe.cuh), slower than the two-kernel path today
+    bool allow_split = false;       // option "split": FIR + first transform stage / 256-point transforms per warp (fe_split.cuh); measured slower
+    float2 *d_sp_tw1 = nullptr, *d_sp_tw256 = nullptr;   // its twiddle tables
+    bool split_attr[3] = {};        // shared-memory attribute set (producer, consumer int8, consumer f32)
     int ring_rows = 32;             // option "ring_rows" (D: rows per track, a power of two >= 16)
     int opt_fir_warps = 0;          // option "fir_warps" (FIR warps per CTA, 0 = as many as the block allows)
     int opt_tracks = 0;             // option "tracks" (J, 0 = as many as the FIR warps serve)
@@ -194,6 +198,32 @@ bool use_tiled(const fengine *fe)
 bool use_fused(const fengine *fe)
 {
     return use_packed(fe) && fe->allow_fused && fe->bits == 10 && (fe->T == 2 || fe->T == 4 || fe->T == 8 || fe->T == 16);
+}
+
+bool use_split(const fengine *fe)
+{
+    return use_packed(fe) && fe->allow_split && fe->bits == 10 && fe->d_sp_tw1 && split_supported(fe->n, fe->T);
+}
+
+// Rows per producer tile of the split path: one CTA per SM, so the tile count is chosen for whole waves over the SMs
+// against the T - 1 warm-up rows every tile pays.
+int split_rows_for(const fengine *fe, int64_t S)
+{
+    if (fe->fir_rows > 0) return fe->fir_rows;
+    const int64_t cols = (int64_t)(fe->n / kSubM) * fe->A;
+    double best = -1.0;
+    int best_rows = (int)S;
+    for (int tiles = 1; tiles <= 64 && tiles <= S; ++tiles) {
+        const int64_t rows = (S + tiles - 1) / tiles;
+        const int64_t ctas = cols * ((S + rows - 1) / rows);
+        const int64_t waves = (ctas + fe->n_sms - 1) / fe->n_sms;
+        const double eff = (double)ctas / (double)(waves * fe->n_sms) * (double)rows / (double)(rows + fe->T - 1);
+        if (eff > best) {
+            best = eff;
+            best_rows = (int)rows;
+        }
+    }
+    return best_rows;
 }
 
 // ---- pipelined kernel: work decomposition of a call (fe_pipe.cuh) ----
@@ -411,10 +441,20 @@ GenParams gen_params(const fengine *fe, const void *in, int64_t S)
 
 unsigned gen_grid(const fengine *fe, int64_t total) { return (unsigned)std::min<int64_t>((total + 255) / 256, (int64_t)fe->n_sms * 16); }
 
+// every entry point runs on the device the handle was created on
+int check_device(fengine *fe)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != fe->device)
+        return fail(fe, FENGINE_ERR_STATE, "handle belongs to device %d, current device is %d", fe->device, dev);
+    return FENGINE_OK;
+}
+
 int check_call(fengine *fe, const void *in, const void *out, int64_t S)
 {
     if (!fe) return FENGINE_ERR_INVALID_ARG;
     fe->err.clear();
+    if (int rc = check_device(fe)) return rc;
     if (S < 0) return fail(fe, FENGINE_ERR_INVALID_ARG, "n_spectra < 0");
     if (S == 0) return FENGINE_OK;
     if (!in || !out) return fail(fe, FENGINE_ERR_INVALID_ARG, "null device pointer");
@@ -426,6 +466,29 @@ int check_call(fengine *fe, const void *in, const void *out, int64_t S)
     if (fe->n_fine != 1 && fe->n_fine < S)
         return fail(fe, FENGINE_ERR_STATE, "fine delay table has %lld entries per stream, need %lld",
                     (long long)fe->n_fine, (long long)S);
+    return FENGINE_OK;
+}
+
+// The rotation x gain tables depend only on what the setters change, so they are rebuilt there, on the legacy stream,
+// and the setter returns after the device has finished: fengine_process never launches a table kernel and a call on
+// any stream (blocking or not) sees complete tables.
+int refresh_tables(fengine *fe)
+{
+    const int streams = fe->A * fe->P;
+    const bool per_spectrum = fe->n_coarse != 1 || fe->n_fine != 1;
+    if (!per_spectrum) {
+        dim3 grid((unsigned)((fe->n + 255) / 256), (unsigned)streams);
+        build_rg_table<<<grid, 256>>>(fe->d_rg, fe->d_gains, fe->d_coarse, fe->d_fine_d, fe->d_fine_phi, fe->n, streams);
+    }
+    if (fe->d_rg2) {
+        const int mode = per_spectrum ? 1 : 0;
+        dim3 grid((unsigned)((fe->n + 255) / 256), (unsigned)fe->A);
+        build_rg2_table<<<grid, 256>>>(fe->d_rg2, fe->d_gains, fe->d_coarse, fe->d_fine_d, fe->d_fine_phi, fe->n, fe->A, mode);
+        fe->rg2_mode = mode;
+    }
+    FE_CUDA(fe, cudaGetLastError());
+    FE_CUDA(fe, cudaDeviceSynchronize());
+    fe->rg_dirty = false;
     return FENGINE_OK;
 }
 
@@ -457,16 +520,11 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
     }
 
     const bool per_spectrum = fe->n_coarse != 1 || fe->n_fine != 1;
-    if (!per_spectrum && fe->rg_dirty) {
-        dim3 grid((unsigned)((fe->n + 255) / 256), (unsigned)streams);
-        build_rg_table<<<grid, 256, 0, stream>>>(fe->d_rg, fe->d_gains, fe->d_coarse, fe->d_fine_d, fe->d_fine_phi,
-                                                fe->n, streams);
-        fe->rg_dirty = false;
-        ++fe->last_launches;
-    }
+    if (fe->rg_dirty) return fail(fe, FENGINE_ERR_STATE, "rotation / gain tables are stale (a setter failed)");
 
     const int64_t chunk = fe->chunk_spectra > 0 ? std::min<int64_t>(fe->chunk_spectra, m_hi - m_lo) : m_hi - m_lo;
     const bool fused = use_fused(fe);
+    const bool split = !fused && use_split(fe);
 
     int rc = fused ? FENGINE_OK : ensure_scratch(fe, (size_t)streams * chunk * fe->N);
     if (rc) return rc;
@@ -524,14 +582,6 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
         xp2.tw1 = fe->d_tw1s;
         xp2.tw2 = fe->d_tw2s;
         xp2.tpost = fe->d_tpost;
-        const int mode = per_spectrum ? 1 : 0;
-        if (fe->rg2_mode != mode) {
-            dim3 grid((unsigned)((fe->n + 255) / 256), (unsigned)fe->A);
-            build_rg2_table<<<grid, 256, 0, stream>>>(fe->d_rg2, fe->d_gains, fe->d_coarse, fe->d_fine_d, fe->d_fine_phi,
-                                                     fe->n, fe->A, mode);
-            fe->rg2_mode = mode;
-            ++fe->last_launches;
-        }
         xp2.rg2 = fe->d_rg2;
         xp2.coarse = fe->d_coarse;
         xp2.fine_d = fe->d_fine_d;
@@ -608,6 +658,26 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
             }
             FE_CUDA(fe, cudaEventRecord(ev[0], stream));
         }
+        if (split) {
+            SplitParams sp{};
+            sp.fir = fp2;
+            sp.fft = xp2;
+            sp.fir.rows_per_tile = split_rows_for(fe, m1 - m0);
+            sp.tw1 = fe->d_sp_tw1;
+            sp.tw256 = fe->d_sp_tw256;
+            const dim3 gridp((unsigned)(fe->n / kSubM), (unsigned)((m1 - m0 + sp.fir.rows_per_tile - 1) / sp.fir.rows_per_tile), (unsigned)fe->A);
+            cudaError_t ce = split_launch_fir(fe->T, fe->n, sp, gridp, !fe->split_attr[0], stream);
+            fe->split_attr[0] = true;
+            if (ce != cudaSuccess) return fail(fe, FENGINE_ERR_CUDA, "split producer launch failed: %s", cudaGetErrorString(ce));
+            if (fe->profile) FE_CUDA(fe, cudaEventRecord(ev[1], stream));
+            bool &attr = fe->split_attr[out_f32 ? 2 : 1];
+            ce = split_launch_fft(fe->n, out_f32 != nullptr, sp, dim3((unsigned)(m1 - m0), (unsigned)fe->A), !attr, stream);
+            attr = true;
+            if (ce != cudaSuccess) return fail(fe, FENGINE_ERR_CUDA, "split consumer launch failed: %s", cudaGetErrorString(ce));
+            if (fe->profile) FE_CUDA(fe, cudaEventRecord(ev[2], stream));
+            fe->last_launches += 2;
+            continue;
+        }
         rc = packed ? launch_fir2(fe, fp2, m1 - m0, stream) : launch_fir(fe, fp, m1 - m0, stream);
         if (rc) return rc;
         if (fe->profile) FE_CUDA(fe, cudaEventRecord(ev[1], stream));
@@ -628,7 +698,7 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
 extern "C" {
 
 fengine_t *fengine_create_batched(int n_antennas, int n_channels, int taps, int n_pols, const float *weights)
-{
+try {
     if (n_antennas < 1 || n_channels < 8 || n_channels > 32768 || (n_channels & (n_channels - 1)) || taps < 1 ||
         taps > 32 || (n_pols != 1 && n_pols != 2) || !weights)
         return nullptr;
@@ -652,6 +722,7 @@ fengine_t *fengine_create_batched(int n_antennas, int n_channels, int taps, int 
     {
         int dev = 0;
         cudaGetDevice(&dev);
+        fe->device = dev;
         cudaDeviceGetAttribute(&fe->n_sms, cudaDevAttrMultiProcessorCount, dev);
         if (fe->n_sms < 1) fe->n_sms = 148;
     }
@@ -689,15 +760,31 @@ fengine_t *fengine_create_batched(int n_antennas, int n_channels, int taps, int 
             case 8192: rc = build_tables2<Plan2_8192>(fe); break;
             }
         }
+        if (rc == FENGINE_OK && fe->packed_ok && split_supported(fe->n, fe->T)) {
+            const int K1 = fe->n / kSubM;
+            if (cudaMalloc(&fe->d_sp_tw1, sizeof(float2) * (size_t)K1 * kSubM) == cudaSuccess &&
+                cudaMalloc(&fe->d_sp_tw256, sizeof(float2) * 256) == cudaSuccess) {
+                build_scalar_twiddles<<<(K1 * kSubM + 255) / 256, 256>>>(fe->d_sp_tw1, K1, kSubM, fe->n);
+                build_scalar_twiddles<<<1, 256>>>(fe->d_sp_tw256, 16, 16, 256);
+                if (cudaGetLastError() != cudaSuccess) rc = FENGINE_ERR_CUDA;
+            } else {
+                rc = FENGINE_ERR_ALLOC;
+            }
+        }
         ok = rc == FENGINE_OK;
     }
     if (ok) ok = cudaDeviceSynchronize() == cudaSuccess;
+    if (ok) ok = refresh_tables(fe) == FENGINE_OK;
     if (!ok) {
         cudaGetLastError();
         fengine_destroy(fe);
         return nullptr;
     }
     return fe;
+} catch (const std::bad_alloc &) {
+    return nullptr;
+} catch (...) {
+    return nullptr;
 }
 
 fengine_t *fengine_create(int n_channels, int taps, int n_pols, const float *weights)
@@ -720,6 +807,8 @@ void fengine_destroy(fengine_t *fe)
     cudaFree(fe->d_tw1s);
     cudaFree(fe->d_tw2s);
     cudaFree(fe->d_rg2);
+    cudaFree(fe->d_sp_tw1);
+    cudaFree(fe->d_sp_tw256);
     cudaFree(fe->d_scratch);
     cudaFree(fe->d_ring);
     cudaFree(fe->d_ctl);
@@ -740,7 +829,7 @@ void fengine_destroy(fengine_t *fe)
 }
 
 int fengine_set_coarse_delays(fengine_t *fe, const int32_t *c, int64_t n_per_stream)
-{
+try {
     if (!fe) return FENGINE_ERR_INVALID_ARG;
     fe->err.clear();
     if (!c || n_per_stream < 1) return fail(fe, FENGINE_ERR_INVALID_ARG, "bad coarse delay table");
@@ -775,12 +864,15 @@ int fengine_set_coarse_delays(fengine_t *fe, const int32_t *c, int64_t n_per_str
             fe->pols_equal = memcmp(c + (size_t)(2 * a) * n_per_stream, c + (size_t)(2 * a + 1) * n_per_stream,
                                     sizeof(int32_t) * (size_t)n_per_stream) == 0;
     fe->rg_dirty = true;
-    fe->rg2_mode = -1;
-    return FENGINE_OK;
+    return refresh_tables(fe);
+} catch (const std::bad_alloc &) {
+    return fail(fe, FENGINE_ERR_ALLOC, "out of host memory");
+} catch (...) {
+    return fail(fe, FENGINE_ERR_CUDA, "unexpected C++ exception");
 }
 
 int fengine_set_fine_delays(fengine_t *fe, const float *delay, const float *phase, int64_t n_per_stream)
-{
+try {
     if (!fe) return FENGINE_ERR_INVALID_ARG;
     fe->err.clear();
     if (!delay || !phase || n_per_stream < 1) return fail(fe, FENGINE_ERR_INVALID_ARG, "bad fine delay table");
@@ -804,12 +896,15 @@ int fengine_set_fine_delays(fengine_t *fe, const float *delay, const float *phas
     FE_CUDA(fe, cudaMemcpy(fe->d_fine_d, delay, sizeof(float) * count, cudaMemcpyHostToDevice));
     FE_CUDA(fe, cudaMemcpy(fe->d_fine_phi, phase, sizeof(float) * count, cudaMemcpyHostToDevice));
     fe->rg_dirty = true;
-    fe->rg2_mode = -1;
-    return FENGINE_OK;
+    return refresh_tables(fe);
+} catch (const std::bad_alloc &) {
+    return fail(fe, FENGINE_ERR_ALLOC, "out of host memory");
+} catch (...) {
+    return fail(fe, FENGINE_ERR_CUDA, "unexpected C++ exception");
 }
 
 int fengine_set_gains(fengine_t *fe, const float *gains_re_im)
-{
+try {
     if (!fe) return FENGINE_ERR_INVALID_ARG;
     fe->err.clear();
     if (!gains_re_im) return fail(fe, FENGINE_ERR_INVALID_ARG, "null gains");
@@ -818,20 +913,27 @@ int fengine_set_gains(fengine_t *fe, const float *gains_re_im)
     FE_CUDA(fe, cudaDeviceSynchronize());
     FE_CUDA(fe, cudaMemcpy(fe->d_gains, gains_re_im, sizeof(float2) * count, cudaMemcpyHostToDevice));
     fe->rg_dirty = true;
-    fe->rg2_mode = -1;
-    return FENGINE_OK;
+    return refresh_tables(fe);
+} catch (const std::bad_alloc &) {
+    return fail(fe, FENGINE_ERR_ALLOC, "out of host memory");
+} catch (...) {
+    return fail(fe, FENGINE_ERR_CUDA, "unexpected C++ exception");
 }
 
 int fengine_process(fengine_t *fe, const void *in, void *out, int64_t n_spectra, void *stream)
-{
+try {
     int rc = check_call(fe, in, out, n_spectra);
     if (rc) return rc;
     if (fe->stream_off != 0) return fail(fe, FENGINE_ERR_STATE, "a stream is open: use fengine_stream_push or fengine_stream_end");
     return process_impl(fe, in, static_cast<int8_t *>(out), nullptr, n_spectra, static_cast<cudaStream_t>(stream));
+} catch (const std::bad_alloc &) {
+    return fail(fe, FENGINE_ERR_ALLOC, "out of host memory");
+} catch (...) {
+    return fail(fe, FENGINE_ERR_CUDA, "unexpected C++ exception");
 }
 
 int fengine_reserve(fengine_t *fe, int64_t max_spectra)
-{
+try {
     if (!fe) return FENGINE_ERR_INVALID_ARG;
     fe->err.clear();
     if (max_spectra < 1) return fail(fe, FENGINE_ERR_INVALID_ARG, "max_spectra < 1");
@@ -848,10 +950,14 @@ int fengine_reserve(fengine_t *fe, int64_t max_spectra)
     FE_CUDA(fe, cudaDeviceSynchronize());
     fe->reserved = true;
     return FENGINE_OK;
+} catch (const std::bad_alloc &) {
+    return fail(fe, FENGINE_ERR_ALLOC, "out of host memory");
+} catch (...) {
+    return fail(fe, FENGINE_ERR_CUDA, "unexpected C++ exception");
 }
 
 int fengine_process_heaps(fengine_t *fe, const void *in, void *heaps_out, int64_t n_spectra, void *stream)
-{
+try {
     int rc = check_call(fe, in, heaps_out, n_spectra);
     if (rc || n_spectra == 0) return rc;
     if (fe->stream_off != 0) return fail(fe, FENGINE_ERR_STATE, "a stream is open: use fengine_stream_push or fengine_stream_end");
@@ -884,6 +990,10 @@ int fengine_process_heaps(fengine_t *fe, const void *in, void *heaps_out, int64_
     ++fe->last_launches;
     FE_CUDA(fe, cudaGetLastError());
     return FENGINE_OK;
+} catch (const std::bad_alloc &) {
+    return fail(fe, FENGINE_ERR_ALLOC, "out of host memory");
+} catch (...) {
+    return fail(fe, FENGINE_ERR_CUDA, "unexpected C++ exception");
 }
 
 // ---- streaming: consecutive pushes continue one sample stream -------------------------------
@@ -897,12 +1007,13 @@ int upload_coarse(fengine *fe)
     for (size_t i = 0; i < count; ++i)
         eff[i] = (int32_t)((int64_t)(i < fe->h_coarse.size() ? fe->h_coarse[i] : 0) - fe->stream_off * fe->N);
     FE_CUDA(fe, cudaMemcpy(fe->d_coarse, eff.data(), sizeof(int32_t) * count, cudaMemcpyHostToDevice));
+    FE_CUDA(fe, cudaDeviceSynchronize());                   // a pageable copy may return before the DMA has landed
     return FENGINE_OK;
 }
 }  // namespace
 
 int fengine_stream_begin(fengine_t *fe, int64_t max_new_spectra, int64_t *delay_out)
-{
+try {
     if (!fe) return FENGINE_ERR_INVALID_ARG;
     fe->err.clear();
     if (max_new_spectra < 1) return fail(fe, FENGINE_ERR_INVALID_ARG, "max_new_spectra < 1");
@@ -933,14 +1044,16 @@ int fengine_stream_begin(fengine_t *fe, int64_t max_new_spectra, int64_t *delay_
     fe->stream_off = back;
     int rc = upload_coarse(fe);
     if (rc) return rc;
-    fe->rg_dirty = true;
-    fe->rg2_mode = -1;
     if (delay_out) *delay_out = fe->win_delay;
     return FENGINE_OK;
+} catch (const std::bad_alloc &) {
+    return fail(fe, FENGINE_ERR_ALLOC, "out of host memory");
+} catch (...) {
+    return fail(fe, FENGINE_ERR_CUDA, "unexpected C++ exception");
 }
 
 int fengine_stream_push(fengine_t *fe, const void *in_new, void *out, int64_t n_new, void *stream)
-{
+try {
     int rc = check_call(fe, in_new, out, n_new);
     if (rc || n_new == 0) return rc;
     if (fe->stream_off == 0) return fail(fe, FENGINE_ERR_STATE, "no stream is open (fengine_stream_begin)");
@@ -963,21 +1076,27 @@ int fengine_stream_push(fengine_t *fe, const void *in_new, void *out, int64_t n_
     fe->win_cur = nxt;
     fe->win_prev_new = n_new;
     return rc;
+} catch (const std::bad_alloc &) {
+    return fail(fe, FENGINE_ERR_ALLOC, "out of host memory");
+} catch (...) {
+    return fail(fe, FENGINE_ERR_CUDA, "unexpected C++ exception");
 }
 
 int fengine_stream_end(fengine_t *fe)
-{
+try {
     if (!fe) return FENGINE_ERR_INVALID_ARG;
     fe->err.clear();
     FE_CUDA(fe, cudaDeviceSynchronize());
     fe->stream_off = 0;
-    fe->rg_dirty = true;
-    fe->rg2_mode = -1;
     return upload_coarse(fe);
+} catch (const std::bad_alloc &) {
+    return fail(fe, FENGINE_ERR_ALLOC, "out of host memory");
+} catch (...) {
+    return fail(fe, FENGINE_ERR_CUDA, "unexpected C++ exception");
 }
 
 int fengine_process_host(fengine_t *fe, const void *in_host, void *out_host, int64_t n_spectra)
-{
+try {
     if (!fe) return FENGINE_ERR_INVALID_ARG;
     fe->err.clear();
     if (n_spectra < 0) return fail(fe, FENGINE_ERR_INVALID_ARG, "n_spectra < 0");
@@ -1066,31 +1185,45 @@ int fengine_process_host(fengine_t *fe, const void *in_host, void *out_host, int
     FE_CUDA(fe, cudaMemcpyAsync(out_host, fe->d_stage_out, out_bytes, cudaMemcpyDeviceToHost, fe->host_stream));
     FE_CUDA(fe, cudaStreamSynchronize(fe->host_stream));
     return FENGINE_OK;
+} catch (const std::bad_alloc &) {
+    return fail(fe, FENGINE_ERR_ALLOC, "out of host memory");
+} catch (...) {
+    return fail(fe, FENGINE_ERR_CUDA, "unexpected C++ exception");
 }
 
 int fengine_process_f32(fengine_t *fe, const void *in, float *spectra_out, int64_t n_spectra, void *stream)
-{
+try {
     int rc = check_call(fe, in, spectra_out, n_spectra);
     if (rc) return rc;
     if (fe->stream_off != 0) return fail(fe, FENGINE_ERR_STATE, "a stream is open: use fengine_stream_push or fengine_stream_end");
     return process_impl(fe, in, nullptr, spectra_out, n_spectra, static_cast<cudaStream_t>(stream));
+} catch (const std::bad_alloc &) {
+    return fail(fe, FENGINE_ERR_ALLOC, "out of host memory");
+} catch (...) {
+    return fail(fe, FENGINE_ERR_CUDA, "unexpected C++ exception");
 }
 
 int fengine_debug_unpack(fengine_t *fe, const void *in, int16_t *samples_out, int64_t n_spectra, void *stream)
-{
+try {
     int rc = check_call(fe, in, samples_out, n_spectra);
     if (rc || n_spectra == 0) return rc;
+    if (fe->stream_off != 0) return fail(fe, FENGINE_ERR_STATE, "a stream is open: the debug hooks see the shifted delay table");
     const GenParams gp = gen_params(fe, in, n_spectra);
     const int64_t total = (int64_t)fe->A * fe->P * n_spectra * fe->N * fe->T;
     gen_unpack_kernel<<<gen_grid(fe, total), 256, 0, static_cast<cudaStream_t>(stream)>>>(gp, samples_out);
     FE_CUDA(fe, cudaGetLastError());
     return FENGINE_OK;
+} catch (const std::bad_alloc &) {
+    return fail(fe, FENGINE_ERR_ALLOC, "out of host memory");
+} catch (...) {
+    return fail(fe, FENGINE_ERR_CUDA, "unexpected C++ exception");
 }
 
 int fengine_debug_fir(fengine_t *fe, const void *in, float *g_out, int64_t n_spectra, void *stream)
-{
+try {
     int rc = check_call(fe, in, g_out, n_spectra);
     if (rc || n_spectra == 0) return rc;
+    if (fe->stream_off != 0) return fail(fe, FENGINE_ERR_STATE, "a stream is open: the debug hooks see the shifted delay table");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const int64_t total = (int64_t)fe->A * fe->P * n_spectra * fe->N;
     if (!use_tiled(fe)) {
@@ -1139,14 +1272,21 @@ int fengine_debug_fir(fengine_t *fe, const void *in, float *g_out, int64_t n_spe
     }
     FE_CUDA(fe, cudaGetLastError());
     return FENGINE_OK;
+} catch (const std::bad_alloc &) {
+    return fail(fe, FENGINE_ERR_ALLOC, "out of host memory");
+} catch (...) {
+    return fail(fe, FENGINE_ERR_CUDA, "unexpected C++ exception");
 }
 
 const char *fengine_last_error(const fengine_t *fe) { return fe ? fe->err.c_str() : "null handle"; }
 
 int fengine_set_option(fengine_t *fe, const char *key, int64_t value)
-{
+try {
     if (!fe || !key) return FENGINE_ERR_INVALID_ARG;
     fe->err.clear();
+    if (fe->stream_off != 0 && (!strcmp(key, "sample_bits") || !strcmp(key, "force_generic") || !strcmp(key, "pol_packed") ||
+                                !strcmp(key, "fused") || !strcmp(key, "split")))
+        return fail(fe, FENGINE_ERR_STATE, "option %s changes the data layout or the path and cannot change while a stream is open", key);
     if (!strcmp(key, "chunk_spectra")) {
         if (value < 0) return fail(fe, FENGINE_ERR_INVALID_ARG, "chunk_spectra < 0");
         fe->chunk_spectra = value;
@@ -1180,6 +1320,10 @@ int fengine_set_option(fengine_t *fe, const char *key, int64_t value)
         fe->allow_fused = value != 0;
         return FENGINE_OK;
     }
+    if (!strcmp(key, "split")) {
+        fe->allow_split = value != 0;
+        return FENGINE_OK;
+    }
     if (!strcmp(key, "ring_rows")) {
         if (value < 16 || value > 4096) return fail(fe, FENGINE_ERR_INVALID_ARG, "ring_rows out of range");
         fe->ring_rows = (int)value;
@@ -1207,10 +1351,14 @@ int fengine_set_option(fengine_t *fe, const char *key, int64_t value)
         return FENGINE_OK;
     }
     return fail(fe, FENGINE_ERR_INVALID_ARG, "unknown option %s", key);
+} catch (const std::bad_alloc &) {
+    return fail(fe, FENGINE_ERR_ALLOC, "out of host memory");
+} catch (...) {
+    return fail(fe, FENGINE_ERR_CUDA, "unexpected C++ exception");
 }
 
 int fengine_profile_read(fengine_t *fe, double *fir_ms, double *fft_ms, int64_t *n_fir, int64_t *n_fft)
-{
+try {
     if (!fe) return FENGINE_ERR_INVALID_ARG;
     fe->err.clear();
     double fir = 0.0, fft = 0.0;
@@ -1231,6 +1379,10 @@ int fengine_profile_read(fengine_t *fe, double *fir_ms, double *fft_ms, int64_t 
     if (n_fir) *n_fir = count;
     if (n_fft) *n_fft = count;
     return FENGINE_OK;
+} catch (const std::bad_alloc &) {
+    return fail(fe, FENGINE_ERR_ALLOC, "out of host memory");
+} catch (...) {
+    return fail(fe, FENGINE_ERR_CUDA, "unexpected C++ exception");
 }
 
 int64_t fengine_last_launch_count(const fengine_t *fe) { return fe ? fe->last_launches : 0; }
@@ -1245,6 +1397,39 @@ int fengine_debug_pipe_stats(fengine_t *fe, uint64_t *out, int64_t max_words)
     FE_CUDA(fe, cudaMemcpy(out, fe->d_stats, sizeof(uint64_t) * (size_t)words, cudaMemcpyDeviceToHost));
     FE_CUDA(fe, cudaMemset(fe->d_stats, 0, sizeof(unsigned long long) * kStCount * (size_t)fe->n_sms));
     return FENGINE_OK;
+}
+
+int fengine_debug_fp32_rate(double *lane_ops_per_second, double *ms_out)
+{
+    if (!lane_ops_per_second) return FENGINE_ERR_INVALID_ARG;
+    int dev = 0, n_sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n_sms < 1) {
+        cudaGetLastError();
+        return FENGINE_ERR_CUDA;
+    }
+    float *out = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    int rc = FENGINE_ERR_CUDA;
+    const int reps = 8;
+    if (cudaMalloc(&out, sizeof(float) * 1024 * (size_t)n_sms) == cudaSuccess && cudaEventCreate(&e0) == cudaSuccess &&
+        cudaEventCreate(&e1) == cudaSuccess) {
+        fp32_rate_kernel<<<n_sms, 1024>>>(out, 1.0f, 0.5f);           // warm-up
+        cudaEventRecord(e0);
+        for (int r = 0; r < reps; ++r) fp32_rate_kernel<<<n_sms, 1024>>>(out, 1.0f, 0.5f);
+        cudaEventRecord(e1);
+        float ms = 0.f;
+        if (cudaEventSynchronize(e1) == cudaSuccess && cudaEventElapsedTime(&ms, e0, e1) == cudaSuccess && ms > 0.f) {
+            const double lane_ops = (double)reps * n_sms * 1024.0 * kRateIters * 16.0 * 2.0;
+            *lane_ops_per_second = lane_ops / (ms * 1e-3);
+            if (ms_out) *ms_out = ms / reps;
+            rc = FENGINE_OK;
+        }
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(out);
+    cudaGetLastError();
+    return rc;
 }
 
 }  // extern "C"

@@ -12,6 +12,21 @@ def shard_antennas(n_antennas: int, world: int, rank: int) -> range:
     return range(start, start + base + (1 if rank < extra else 0))
 
 
+def rank_slice(world: int, rank: int, packed, coarse, fine_delay, phase, gains) -> dict:
+    """What one rank builds its engine from: the contiguous antenna block of every per-antenna array (antenna is the
+    outermost index of all of them and of in / out, include/fengine.h), plus `n_antennas` and the block itself.
+    The weights are replicated, not sliced."""
+    import numpy as np
+    block = shard_antennas(int(packed.shape[0]), world, rank)
+    sl = slice(block.start, block.stop)
+    for name, arr in (("coarse", coarse), ("fine_delay", fine_delay), ("phase", phase), ("gains", gains)):
+        if arr.shape[0] != packed.shape[0]:
+            raise ValueError(f"{name}: antenna must be the outermost index")
+    return dict(n_antennas=len(block), antennas=block, packed=np.ascontiguousarray(packed[sl]),
+                coarse=np.ascontiguousarray(coarse[sl]), fine_delay=np.ascontiguousarray(fine_delay[sl]),
+                phase=np.ascontiguousarray(phase[sl]), gains=np.ascontiguousarray(gains[sl]))
+
+
 def max_over_ranks(value: float, dist=None, device=None) -> float:
     """Max of a timing scalar over the ranks of the default process group (the only collective of the job)."""
     if dist is None or not dist.is_available() or not dist.is_initialized() or dist.get_world_size() == 1:

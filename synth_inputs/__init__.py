@@ -218,14 +218,24 @@ def make_workload(config: int, n_spectra: int | None = None, n_antennas: int | N
     scale = 2.0 ** (bits - 10)
     packed = np.empty((A, P, L * bits // 8), dtype=np.uint8)
     samples = np.empty((A, P, L), dtype=np.int16) if keep_samples else None
-    for a in range(A):
-        for p in range(P):
-            rng = np.random.default_rng([seed, config, a, p])
-            tn = tones[a] if bits == 10 else [(k, amp * scale, th) for (k, amp, th) in tones[a]]
-            s = _samples(rng, L, N, sig * scale, tn, bits)      # tone common to both pols, independent noise
-            packed[a, p] = pack_bits(s, bits)
-            if keep_samples:
-                samples[a, p] = s
+    def one_stream(ap):
+        a, p = ap
+        rng = np.random.default_rng([seed, config, a, p])       # one generator per stream: the result does not depend
+        tn = tones[a] if bits == 10 else [(k, amp * scale, th) for (k, amp, th) in tones[a]]      # on the thread count
+        s = _samples(rng, L, N, sig * scale, tn, bits)          # tone common to both pols, independent noise
+        packed[a, p] = pack_bits(s, bits)
+        if keep_samples:
+            samples[a, p] = s
+
+    streams = [(a, p) for a in range(A) for p in range(P)]
+    if L * len(streams) >= 1 << 24:                             # large batches: numpy releases the GIL in these loops
+        from concurrent.futures import ThreadPoolExecutor
+        import os
+        with ThreadPoolExecutor(max_workers=min(len(streams), os.cpu_count() or 1)) as ex:
+            list(ex.map(one_stream, streams))
+    else:
+        for ap in streams:
+            one_stream(ap)
     return Workload(name=f"config{config}", A=A, P=P, n=n, T=T, S=S, packed=packed, weights=weights,
                     coarse=np.ascontiguousarray(coarse), fine_delay=np.ascontiguousarray(fine),
                     phase=np.ascontiguousarray(phase), gains=gains, samples=samples,

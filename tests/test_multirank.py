@@ -28,9 +28,16 @@ def _worker(rank, world, port, A, out_dir):
         w = si.custom_workload(A=A, n=64, T=4, S=6, P=2, seed=5, random_weights=True, coarse_range=(-10, 200))
         mine = sharding.shard_antennas(A, world, rank)
         sel = list(mine)
+        # the product-side slicing: exactly what a rank hands to FEngine(...) / the setters / fengine_process
+        rs = sharding.rank_slice(world, rank, w.packed, w.coarse, w.fine_delay, w.phase, w.gains)
+        assert rs["n_antennas"] == len(sel) and list(rs["antennas"]) == sel
+        for key, full in (("packed", w.packed), ("coarse", w.coarse), ("fine_delay", w.fine_delay), ("phase", w.phase),
+                          ("gains", w.gains)):
+            assert rs[key].flags["C_CONTIGUOUS"] and rs[key].dtype == full.dtype
+            np.testing.assert_array_equal(rs[key], full[sel])
         # each rank runs the path on its own antennas only (here: the oracle stands in for the GPU, CPU test)
-        res = oracle.process(w.packed[sel], len(sel), w.n, w.T, w.P, w.weights, w.S, coarse=w.coarse[sel],
-                             fine_delay=w.fine_delay[sel], phase=w.phase[sel], gains=w.gains[sel])
+        res = oracle.process(rs["packed"], rs["n_antennas"], w.n, w.T, w.P, w.weights, w.S, coarse=rs["coarse"],
+                             fine_delay=rs["fine_delay"], phase=rs["phase"], gains=rs["gains"])
         np.save(os.path.join(out_dir, f"out_{rank}.npy"), res["out"])
         t = sharding.max_over_ranks(1.0 + rank, dist)            # slowest rank decides
         assert t == float(world)
