@@ -214,6 +214,19 @@ int64_t fengine_last_launch_count(const fengine_t *fe);
  * ([n_sms][16] uint64) and zeroes them.  Synchronises the device. */
 int fengine_debug_pipe_stats(fengine_t *fe, uint64_t *out, int64_t max_words);
 
+/* Which kernels fengine_process would launch now (options, shape, equal or unequal coarse delays of the two pols):
+ * a test hook, so that a parity test of a shape can assert that it exercised the tiled kernels it was written for
+ * (every path computes steps 1-7 of PAPER.md:31-43).  Returns a FENGINE_PATH_* value, -1 for a null handle. */
+enum {
+    FENGINE_PATH_GENERIC = 0,                 /* one thread per output (any shape; slow, for tests) */
+    FENGINE_PATH_ONE_POL = 1,                 /* fe_fir.cuh + fe_fft.cuh */
+    FENGINE_PATH_POL_PACKED = 2,              /* fe_fir2.cuh / fe_fir2b.cuh / fe_fir3.cuh + fe_fft2.cuh */
+    FENGINE_PATH_PACKED_FIR_ONE_POL_FFT = 3,  /* fe_fir2b.cuh / fe_fir3.cuh + fe_fft.cuh (n >= 16384: 32 taps, other sample widths) */
+    FENGINE_PATH_FUSED = 4,                   /* fe_pipe.cuh */
+    FENGINE_PATH_SPLIT = 5                    /* fe_split.cuh */
+};
+int fengine_debug_path(const fengine_t *fe);
+
 /* Measurement hook for the "alu" roofline (BASELINE.json north_star: "the FIR+FFT flops at FP32 peak"; the FIR of
  * Eq. (1), is 2T flops per sample in exactly this instruction form): runs a loop of packed FP32
  * multiply-adds (FFMA2, the FIR kernels' operand pattern) on every SM of the current device, a few launches timed with

@@ -16,7 +16,7 @@ EXPORTED_SYMBOLS = [
     "fengine_set_fine_delays", "fengine_set_gains", "fengine_process", "fengine_process_host",
     "fengine_last_error", "fengine_process_f32", "fengine_debug_unpack", "fengine_debug_fir",
     "fengine_set_option", "fengine_last_launch_count", "fengine_profile_read", "fengine_process_heaps",
-    "fengine_stream_begin", "fengine_stream_push", "fengine_stream_end", "fengine_reserve", "fengine_debug_pipe_stats", "fengine_debug_fp32_rate",
+    "fengine_stream_begin", "fengine_stream_push", "fengine_stream_end", "fengine_reserve", "fengine_debug_pipe_stats", "fengine_debug_fp32_rate", "fengine_debug_path",
 ]
 
 STATUS = {0: "OK", 1: "INVALID_ARG", 2: "ALLOC", 3: "CUDA", 4: "STATE"}
@@ -56,6 +56,7 @@ def lib() -> C.CDLL:
         L.fengine_reserve.argtypes = [vp, i64]
         L.fengine_debug_pipe_stats.argtypes = [vp, vp, i64]
         L.fengine_debug_fp32_rate.argtypes = [vp, vp]
+        L.fengine_debug_path.argtypes = [vp]
         L.fengine_process_heaps.argtypes = [vp, vp, vp, i64, vp]
         L.fengine_stream_begin.argtypes = [vp, i64, vp]
         L.fengine_stream_push.argtypes = [vp, vp, vp, i64, vp]
@@ -259,6 +260,12 @@ class FEngine:
         out = np.zeros((n_sms, 16), dtype=np.uint64)
         self._check(self._lib.fengine_debug_pipe_stats(self._h, _host_ptr(out), out.size))
         return out
+
+    PATHS = {0: "generic", 1: "one_pol", 2: "pol_packed", 3: "packed_fir_one_pol_fft", 4: "fused", 5: "split"}
+
+    def path(self) -> str:
+        """fengine_debug_path: which kernels process() would launch now."""
+        return self.PATHS[int(self._lib.fengine_debug_path(self._h))]
 
     def last_launch_count(self) -> int:
         return int(self._lib.fengine_last_launch_count(self._h))

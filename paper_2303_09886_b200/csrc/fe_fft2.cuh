@@ -56,6 +56,16 @@ struct RowInShared {
     uint32_t s;                 // shared-space address of unit 0
     __device__ __forceinline__ float4 operator()(int i) const { return lds_f4(s + (uint32_t)i * 16u); }
 };
+// The row in the exchange buffer's own layout (block t of M1 units at t * blk): pass 1 then works IN PLACE, thread
+// `col` reads the units (t, col) and writes the units (k, col), the same 16 addresses (persistent kernel below).
+template <class Plan>
+struct RowInPlace {
+    uint32_t s;                 // shared-space address of the buffer
+    __device__ __forceinline__ float4 operator()(int i) const
+    {
+        return lds_f4(s + (uint32_t)(i + i / Plan::M1 * (Plan::blk - Plan::M1)) * 16u);
+    }
+};
 // CTA-wide barrier of the one-spectrum-per-CTA kernels; the pipelined kernel passes a named barrier over its FFT team
 struct SyncCta {
     __device__ __forceinline__ void operator()() const { __syncthreads(); }
@@ -363,11 +373,9 @@ __device__ __forceinline__ void fft2_setup_phase(const Fft2Params &prm, Spectrum
 // the pipelined kernel).  `after_load()` runs (on every thread) once the row has been consumed (after the barrier
 // that ends the last pass 1): the pipelined kernel hands its landing buffer back to the loader there.
 template <class Plan, bool F32OUT, class Row, class Sync, class AfterLoad>
-__device__ __forceinline__ void fft2_row(const Fft2Params &prm, const Row &grow, unsigned char *smem_raw, int a,
-                                         int64_t m, int tid, const Sync &sync, AfterLoad after_load)
+__device__ __forceinline__ void fft2_row_at(const Fft2Params &prm, const Row &grow, float4 *sm, SpectrumPhase2 *sph, int a,
+                                            int64_t m, int tid, const Sync &sync, AfterLoad after_load)
 {
-    float4 *sm = reinterpret_cast<float4 *>(smem_raw);
-    SpectrumPhase2 *sph = reinterpret_cast<SpectrumPhase2 *>(smem_raw + (size_t)Plan::units * 16);
     if (prm.per_spectrum) fft2_setup_phase<Plan>(prm, sph, a, m, tid);
     if constexpr (Plan::SW == 1) {
         fft2_pass1<Plan>(grow, sm, prm.tw1, tid);
@@ -392,6 +400,14 @@ __device__ __forceinline__ void fft2_row(const Fft2Params &prm, const Row &grow,
     }
 }
 
+template <class Plan, bool F32OUT, class Row, class Sync, class AfterLoad>
+__device__ __forceinline__ void fft2_row(const Fft2Params &prm, const Row &grow, unsigned char *smem_raw, int a,
+                                         int64_t m, int tid, const Sync &sync, AfterLoad after_load)
+{
+    fft2_row_at<Plan, F32OUT>(prm, grow, reinterpret_cast<float4 *>(smem_raw),
+                              reinterpret_cast<SpectrumPhase2 *>(smem_raw + (size_t)Plan::units * 16), a, m, tid, sync, after_load);
+}
+
 template <class Plan>
 constexpr size_t fft2_smem_bytes()
 {
@@ -411,6 +427,100 @@ static __global__ void __launch_bounds__(Plan::tpf, (512 / Plan::tpf) > 0 ? (512
     if (m < prm.m_begin) return;
     const RowInGlobal grow{reinterpret_cast<const float4 *>(prm.g + ((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * (int64_t)N * 2)};
     fft2_row<Plan, F32OUT>(prm, grow, smem_raw, a, m, threadIdx.x, SyncCta{}, [] {});
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Persistent variant (one-sweep plans, n <= 4096): one CTA per SM, NT teams of Plan::tpf threads, NT + 1 exchange
+// buffers.  fft2_kernel is latency bound: a CTA waits for the sixteen dependent global loads of pass 1 before it has
+// anything to compute, and only one other CTA of the SM can fill the gap.  Here the rows arrive by bulk copy
+// (cp.async.bulk, the "recent CUDA asynchronous APIs" of PAPER.md:213) straight into the exchange buffer's own
+// skewed layout, so pass 1 runs in place out of shared memory, and they arrive EARLY: the CTA's j-th row lives in
+// buffer j mod (NT + 1) and is transformed by team j mod NT; the team that finishes row j hands the buffer to the
+// copy of row j + NT + 1, which lands while every team is busy with the rows in between.  Teams synchronise among
+// themselves with named barriers and with the copies through one mbarrier per buffer; there is no CTA-wide barrier
+// after the start.  A buffer's rows are handed from team to team (row j + NT + 1 belongs to another team than row
+// j), so a team that runs ahead could meet the buffer's mbarrier two phases early, where a parity wait cannot tell
+// "not yet issued" from "already landed"; the issuing thread therefore also publishes the fill count of the buffer
+// in shared memory and a team waits for "fill k issued" before it waits for the phase k of the mbarrier.
+template <class Plan>
+struct Fft2pSmem {
+    static constexpr int NT = 512 / Plan::tpf;                            // teams per CTA
+    static constexpr int NB = NT + 1;                                     // buffers
+    static constexpr uint32_t buf_bytes = ((uint32_t)Plan::units * 16u + 127u) & ~127u;
+    static constexpr uint32_t sph_off = NB * buf_bytes;
+    static constexpr uint32_t bar_off = sph_off + NT * (((uint32_t)sizeof(SpectrumPhase2) + 15u) & ~15u);
+    static constexpr uint32_t gen_off = bar_off + 8 * NB;                 // int per buffer: fills issued so far - 1
+    static constexpr size_t bytes = gen_off + 4 * NB;
+};
+
+template <class Plan, bool F32OUT>
+static __global__ void __launch_bounds__(512, 1) fft2p_kernel(const __grid_constant__ Fft2Params prm, int A)
+{
+    static_assert(Plan::SW == 1, "in-place landing needs a one-sweep plan");
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    using SM = Fft2pSmem<Plan>;
+    constexpr int NT = SM::NT, NB = SM::NB, tpf = Plan::tpf, N = 2 * Plan::n;
+    constexpr uint32_t blk_bytes = (uint32_t)Plan::M1 * 16u;              // one block of M1 units of the row
+    const int team = threadIdx.x / tpf, tid = threadIdx.x - team * tpf;
+    const uint32_t s_base = smem_u32(smem_raw), bar0 = s_base + SM::bar_off;
+    const int len = (int)(prm.m_end - prm.m_begin), total = len * A;       // the host keeps A * len below 2^31
+    const int c = blockIdx.x, G = gridDim.x;
+
+    // row q of the call, in the reverse of the FIR kernel's write order (the newest scratch rows are still in L2)
+    auto row_ptr = [&](int q, int &a, int64_t &m) {
+        const int ar = q / len, x = q - ar * len;
+        a = A - 1 - (int)ar;
+        m = prm.m_end - 1 - x;
+        return reinterpret_cast<const unsigned char *>(prm.g + ((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * (int64_t)N * 2);
+    };
+    auto issue = [&](int j) {                                         // one thread: row j of this CTA -> buffer j % NB
+        const int q = c + j * G;
+        if (q >= total) return;
+        int a;
+        int64_t m;
+        const unsigned char *src = row_ptr(q, a, m);
+        const int b = j % NB;
+        const uint32_t dst = s_base + (uint32_t)b * SM::buf_bytes, bar = bar0 + 8u * b;
+        fence_proxy_async();                                              // the team's shared-memory accesses before the copy's
+        mbar_arrive_expect_tx(bar, (uint32_t)Plan::R1 * blk_bytes);
+#pragma unroll 1
+        for (int t = 0; t < Plan::R1; ++t) bulk_g2s(dst + (uint32_t)t * (uint32_t)Plan::blk * 16u, src + (size_t)t * blk_bytes, blk_bytes, bar);
+        __threadfence_block();                                            // the mbarrier is armed before the fill count says so
+        asm volatile("st.volatile.shared.s32 [%0], %1;" ::"r"(s_base + SM::gen_off + 4u * b), "r"(j / NB) : "memory");
+    };
+
+    if (threadIdx.x == 0) {
+        for (int b = 0; b < NB; ++b) {
+            mbar_init(bar0 + 8u * b, 1);
+            asm volatile("st.volatile.shared.s32 [%0], %1;" ::"r"(s_base + SM::gen_off + 4u * b), "r"(-1) : "memory");
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (threadIdx.x == 0)
+        for (int j = 0; j < NB; ++j) issue(j);
+
+    SpectrumPhase2 *sph = reinterpret_cast<SpectrumPhase2 *>(smem_raw + SM::sph_off + team * (((uint32_t)sizeof(SpectrumPhase2) + 15u) & ~15u));
+    const auto sync = [team] { bar_sync(1 + team, tpf); };
+    for (int j = team; c + j * G < total; j += NT) {
+        int a;
+        int64_t m;
+        row_ptr(c + j * G, a, m);
+        const int b = j % NB;
+        for (;;) {                                                        // fill j / NB of this buffer has been issued ...
+            int gen;
+            asm volatile("ld.volatile.shared.s32 %0, [%1];" : "=r"(gen) : "r"(s_base + SM::gen_off + 4u * b) : "memory");
+            if (gen >= j / NB) break;
+            __nanosleep(40);
+        }
+        __threadfence_block();
+        mbar_wait(bar0 + 8u * b, (uint32_t)((j / NB) & 1));              // ... and has landed
+        float4 *sm = reinterpret_cast<float4 *>(smem_raw + (size_t)b * SM::buf_bytes);
+        const RowInPlace<Plan> row{s_base + (uint32_t)b * SM::buf_bytes};
+        fft2_row_at<Plan, F32OUT>(prm, row, sm, sph, a, m, tid, sync, [] {});
+        sync();                                                           // every thread of the team is done with the buffer
+        if (tid == 0) issue(j + NB);
+    }
 }
 
 // Pol-interleaved table of the pol-packed epilogue, [A][n] units {re p0, re p1, im p0, im p1}:

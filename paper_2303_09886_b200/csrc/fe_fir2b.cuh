@@ -23,7 +23,10 @@ template <int BITS> struct Fir2Geom {
     static_assert(batch_chunks <= 64, "at most two chunks per lane and batch");
 };
 
-template <int T, bool MIXED, int BITS>
+// ONEPOL: write the scratch in the layout of the one-pol FFT (fe_fft.cuh: a row of N floats per (antenna, spectrum,
+// pol), every four columns stored as (g0, g2, g1, g3)) instead of the pol-packed units: the bit-depth sweep at
+// n = 32768 (Fig. 11), which the pol-packed FFT does not cover, then still runs a tiled FIR.
+template <int T, bool MIXED, int BITS, bool ONEPOL = false>
 __device__ __forceinline__ void fir2b_run(const Fir2Params &prm, const uint8_t *wsrc, uint32_t ring_s, int64_t c,
                                          int64_t m0, int n_out, int i_pt, float *grow0)
 {
@@ -103,7 +106,9 @@ __device__ __forceinline__ void fir2b_run(const Fir2Params &prm, const uint8_t *
     float4 prev = make_float4(0.f, 0.f, 0.f, 0.f);
 
     const size_t g_stride = (size_t)N * 2;                      // next spectrum (floats): n units of 4 floats
-    float *gp = grow0 + 4 * i_pt + ((int64_t)(MIXED ? 0 : lag0) - T) * (int64_t)g_stride;
+    // ONEPOL: grow0 is row (antenna, spectrum, pol 0), pol 1 the next row; point i = 2 q + e holds the columns
+    // 4 q + 2 e (Re z, stored at 4 q + e) and 4 q + 2 e + 1 (Im z, stored at 4 q + 2 + e)
+    float *gp = grow0 + (ONEPOL ? 4 * (i_pt >> 1) + (i_pt & 1) : 4 * i_pt) + ((int64_t)(MIXED ? 0 : lag0) - T) * (int64_t)g_stride;
     int sp = (MIXED ? 0 : lag0) - T;
 
     // The loop is software-pipelined by one step and has no branch in its unrolled body: the raw words of step
@@ -158,8 +163,13 @@ __device__ __forceinline__ void fir2b_run(const Fir2Params &prm, const uint8_t *
                 cur.w = lagc[1] ? prev.w : now.w;
                 prev = now;
             }
-            asm volatile("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %5, %6;\n\t@p st.global.v4.f32 [%0], {%1, %2, %3, %4};\n\t}"
-                         ::"l"(gp), "f"(cur.x), "f"(cur.y), "f"(cur.z), "f"(cur.w), "r"((unsigned)sp), "r"((unsigned)n_out) : "memory");
+            if (ONEPOL)
+                asm volatile("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %6, %7;\n\t@p st.global.f32 [%0], %2;\n\t@p st.global.f32 [%0+8], %4;\n\t"
+                             "@p st.global.f32 [%1], %3;\n\t@p st.global.f32 [%1+8], %5;\n\t}"
+                             ::"l"(gp), "l"(gp + N), "f"(cur.x), "f"(cur.y), "f"(cur.z), "f"(cur.w), "r"((unsigned)sp), "r"((unsigned)n_out) : "memory");
+            else
+                asm volatile("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %5, %6;\n\t@p st.global.v4.f32 [%0], {%1, %2, %3, %4};\n\t}"
+                             ::"l"(gp), "f"(cur.x), "f"(cur.y), "f"(cur.z), "f"(cur.w), "r"((unsigned)sp), "r"((unsigned)n_out) : "memory");
             gp += g_stride;
             ++sp;
         }
@@ -167,7 +177,7 @@ __device__ __forceinline__ void fir2b_run(const Fir2Params &prm, const uint8_t *
     cp_async_wait<0>();
 }
 
-template <int T, int BITS>
+template <int T, int BITS, bool ONEPOL = false>
 __global__ void __launch_bounds__(kFir2Threads, 4) fir2b_kernel(const Fir2Params prm)
 {
     using G = Fir2Geom<BITS>;
@@ -195,9 +205,9 @@ __global__ void __launch_bounds__(kFir2Threads, 4) fir2b_kernel(const Fir2Params
         const int cr = (int)((int64_t)c & (int64_t)(N - 1));
         const bool mixed = (2 * i_pt + cr < N) && (2 * i_pt + 1 + cr >= N);
         if (__any_sync(0xffffffffu, mixed))
-            fir2b_run<T, true, BITS>(prm, wsrc, ring_s, (int64_t)c, m, (int)(run_end - m), i_pt, grow0);
+            fir2b_run<T, true, BITS, ONEPOL>(prm, wsrc, ring_s, (int64_t)c, m, (int)(run_end - m), i_pt, grow0);
         else
-            fir2b_run<T, false, BITS>(prm, wsrc, ring_s, (int64_t)c, m, (int)(run_end - m), i_pt, grow0);
+            fir2b_run<T, false, BITS, ONEPOL>(prm, wsrc, ring_s, (int64_t)c, m, (int)(run_end - m), i_pt, grow0);
         m = run_end;
     }
 }

@@ -22,7 +22,10 @@ constexpr int kFir3SegBytes = 160;                                  // 128 colum
 constexpr int kFir3SlotBytes = 2 * kFir3SegBytes;                   // both pols
 constexpr int kFir3RingBytes = kFirDepth * kFir3SlotBytes + 16;     // +16: the second word of the last thread's group
 
-template <int T>
+// ONEPOL: write the scratch in the layout of the one-pol FFT (fe_fft.cuh: a row of N floats per (antenna, spectrum,
+// pol), every four columns stored as (g0, g2, g1, g3)) instead of the pol-packed units, so that shapes the pol-packed
+// FFT does not cover (n >= 16384) still get a tiled FIR for 32 taps (Fig. 8: "for 32 768 channels").
+template <int T, bool ONEPOL = false>
 __device__ __forceinline__ void fir3_run(const Fir2Params &prm, const uint8_t *csrc, uint32_t ring_s, int64_t c,
                                          int64_t m0, int n_out, int v, float *grow0)
 {
@@ -86,7 +89,9 @@ __device__ __forceinline__ void fir3_run(const Fir2Params &prm, const uint8_t *c
     for (int j = 0; j < T; ++j) acc[j] = f2(0.f, 0.f);
 
     const size_t g_stride = (size_t)N * 2;                        // next spectrum (floats)
-    float *gp = grow0 + 4 * (v >> 1) + 2 * (v & 1) + ((int64_t)lag - T) * (int64_t)g_stride;
+    // ONEPOL: grow0 is row (antenna, spectrum, pol 0); pol 1 is the next row; column v sits at 4 (v / 4) + {0, 2, 1, 3}[v % 4]
+    float *gp = grow0 + (ONEPOL ? 4 * (v >> 2) + (((v & 1) << 1) | ((v >> 1) & 1)) : 4 * (v >> 1) + 2 * (v & 1)) +
+                ((int64_t)lag - T) * (int64_t)g_stride;
     int sp = lag - T;
 
     uint32_t nxt[4];
@@ -113,8 +118,12 @@ __device__ __forceinline__ void fir3_run(const Fir2Params &prm, const uint8_t *c
 #pragma unroll
             for (int j = 1; j < T; ++j) acc[(ii + T - j) % T] = fma_(s, w[j], acc[(ii + T - j) % T]);
             const f2 d = acc[(ii + 1) % T];
-            asm volatile("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %3, %4;\n\t@p st.global.v2.f32 [%0], {%1, %2};\n\t}"
-                         ::"l"(gp), "f"(d.v.x), "f"(d.v.y), "r"((unsigned)sp), "r"((unsigned)n_out) : "memory");
+            if (ONEPOL)
+                asm volatile("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %4, %5;\n\t@p st.global.f32 [%0], %2;\n\t@p st.global.f32 [%1], %3;\n\t}"
+                             ::"l"(gp), "l"(gp + N), "f"(d.v.x), "f"(d.v.y), "r"((unsigned)sp), "r"((unsigned)n_out) : "memory");
+            else
+                asm volatile("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %3, %4;\n\t@p st.global.v2.f32 [%0], {%1, %2};\n\t}"
+                             ::"l"(gp), "f"(d.v.x), "f"(d.v.y), "r"((unsigned)sp), "r"((unsigned)n_out) : "memory");
             gp += g_stride;
             ++sp;
         }
@@ -122,7 +131,7 @@ __device__ __forceinline__ void fir3_run(const Fir2Params &prm, const uint8_t *c
     cp_async_wait<0>();
 }
 
-template <int T>
+template <int T, bool ONEPOL = false>
 __global__ void __launch_bounds__(kFir3Threads, 4) fir3_kernel(const Fir2Params prm)
 {
     __shared__ __align__(16) unsigned char ring_all[kFir3RingBytes];
@@ -143,7 +152,7 @@ __global__ void __launch_bounds__(kFir3Threads, 4) fir3_kernel(const Fir2Params 
             while (run_end < m_stop && ctab[run_end] == c) ++run_end;
         }
         float *grow0 = prm.g + ((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * (int64_t)N * 2;
-        fir3_run<T>(prm, csrc, ring_s, (int64_t)c, m, (int)(run_end - m), v, grow0);
+        fir3_run<T, ONEPOL>(prm, csrc, ring_s, (int64_t)c, m, (int)(run_end - m), v, grow0);
         m = run_end;
     }
 }

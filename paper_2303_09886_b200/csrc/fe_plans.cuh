@@ -19,6 +19,10 @@ using Plan2_2048 = Fft2Plan<2048, 8, 16, 128>;
 using Plan2_4096 = Fft2Plan<4096, 16, 16, 256>;
 using Plan2_8192 = Fft2Plan<8192, 16, 16, 256, 2>;    // two sweeps of 4096 points
 
+// launcher of the persistent pol-packed FFT kernel (fe_fft2p.cu)
+bool fft2p_supported(int n);
+cudaError_t fft2p_launch(int n, bool f32out, const Fft2Params &prm, int A, int grid, bool set_attr, cudaStream_t stream);
+
 // launcher of the pipelined kernel (fe_pipe.cu)
 struct PipeParams;
 int pipe_team_threads(int n);

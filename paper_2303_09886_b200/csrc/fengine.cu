@@ -60,6 +60,10 @@ struct fengine {
     unsigned int *d_ctl = nullptr;
     size_t ctl_words = 0;
     bool allow_fused = false;       // option "fused": the pipelined kernel (fe_pipe.cuh), slower than the two-kernel path today
+    bool l2_persist = false;        // option "l2_persist": launch the two kernels with a persisting L2 window over the scratch
+    cudaAccessPolicyWindow l2_win{};
+    bool allow_fft2p = false;       // option "fft_persistent": persistent pol-packed FFT with bulk-copy prefetch (fft2p_kernel); measured slower
+    bool fft2p_attr[2] = {};
     bool allow_split = false;       // option "split": FIR + first transform stage / 256-point transforms per warp (fe_split.cuh); measured slower
     float2 *d_sp_tw1 = nullptr, *d_sp_tw256 = nullptr;   // its twiddle tables
     bool split_attr[3] = {};        // shared-memory attribute set (producer, consumer int8, consumer f32)
@@ -161,6 +165,27 @@ int build_tables2(fengine *fe)
     return FENGINE_OK;
 }
 
+// kernel launch with an optional persisting-L2 access-policy window (option "l2_persist": the scratch of an L2-sized
+// chunk is rewritten in place chunk after chunk, and lines that persist are not written back in between)
+template <class... KArgs, class... Args>
+cudaError_t launch_win(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream,
+                       const cudaAccessPolicyWindow *win, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute at[1];
+    if (win) {
+        at[0].id = cudaLaunchAttributeAccessPolicyWindow;
+        at[0].val.accessPolicyWindow = *win;
+        cfg.attrs = at;
+        cfg.numAttrs = 1;
+    }
+    return cudaLaunchKernelEx(&cfg, kernel, args...);
+}
+
 template <class Plan, bool F32OUT>
 int launch_fft2(fengine *fe, const Fft2Params &prm, int64_t chunk_len, cudaStream_t stream)
 {
@@ -171,7 +196,10 @@ int launch_fft2(fengine *fe, const Fft2Params &prm, int64_t chunk_len, cudaStrea
         attr_set = true;
     }
     dim3 grid((unsigned)chunk_len, (unsigned)fe->A);
-    fft2_kernel<Plan, F32OUT><<<grid, Plan::tpf, smem, stream>>>(prm);
+    if (fe->l2_persist)
+        FE_CUDA(fe, launch_win(fft2_kernel<Plan, F32OUT>, grid, dim3(Plan::tpf), smem, stream, &fe->l2_win, prm));
+    else
+        fft2_kernel<Plan, F32OUT><<<grid, Plan::tpf, smem, stream>>>(prm);
     return FENGINE_OK;
 }
 
@@ -187,11 +215,18 @@ int launch_fft2_n(fengine *fe, const Fft2Params &prm, int64_t chunk_len, cudaStr
     return fail(fe, FENGINE_ERR_INVALID_ARG, "no pol-packed FFT plan for n=%d", fe->n);
 }
 
-// T = 32 exists only as the one-column pol-packed FIR (fe_fir3.cuh); other 32-tap engines run the generic kernels
-// ... and sample widths other than 10 bits only as the 16-tap pol-packed FIR (fe_fir2.cuh)
+// Shapes the pol-packed FFT does not cover (n >= 16384) but a pol-packed FIR does: 32 taps (fe_fir3.cuh) and sample
+// widths other than 10 bits with 16 taps (fe_fir2b.cuh) write the scratch in the one-pol FFT's layout, so the tap and
+// bit-depth sweeps of the paper (both at 32768 channels) run tiled kernels end to end.
+bool use_packed_fir_onepol_fft(const fengine *fe)
+{
+    if (!fe->tiled || use_packed(fe) || fe->P != 2 || !fe->pols_equal || !fe->allow_packed) return false;
+    return (fe->T == 32 && fe->bits == 10) || (fe->T == 16 && fe->bits != 10);
+}
 bool use_tiled(const fengine *fe)
 {
     if (!fe->tiled) return false;
+    if (use_packed_fir_onepol_fft(fe)) return true;
     if (fe->bits != 10) return use_packed(fe) && fe->T == 16;
     return fe->T != 32 || use_packed(fe);
 }
@@ -312,17 +347,30 @@ int ensure_pipe(fengine *fe, const PipePlan &pl)
     return FENGINE_OK;
 }
 
-int launch_fir2(fengine *fe, const Fir2Params &prm, int64_t chunk_len, cudaStream_t stream)
+int launch_fir2(fengine *fe, const Fir2Params &prm, int64_t chunk_len, cudaStream_t stream, bool onepol = false)
 {
     if (fe->T == 32) {                                      // one column per thread: 32 taps stay in registers
         dim3 grid3((unsigned)(fe->N / kFir3Threads), (unsigned)((chunk_len + prm.rows_per_tile - 1) / prm.rows_per_tile),
                    (unsigned)fe->A);
-        fir3_kernel<32><<<grid3, kFir3Threads, 0, stream>>>(prm);
+        if (onepol)
+            fir3_kernel<32, true><<<grid3, kFir3Threads, 0, stream>>>(prm);
+        else
+            fir3_kernel<32><<<grid3, kFir3Threads, 0, stream>>>(prm);
         return FENGINE_OK;
     }
     dim3 grid((unsigned)(fe->n / kFir2Threads), (unsigned)((chunk_len + prm.rows_per_tile - 1) / prm.rows_per_tile),
               (unsigned)fe->A);
     if (fe->bits != 10) {                                   // bit-depth sweep: 16 taps only
+        if (onepol) {
+            switch (fe->bits) {
+            case 4: fir2b_kernel<16, 4, true><<<grid, kFir2Threads, 0, stream>>>(prm); break;
+            case 8: fir2b_kernel<16, 8, true><<<grid, kFir2Threads, 0, stream>>>(prm); break;
+            case 12: fir2b_kernel<16, 12, true><<<grid, kFir2Threads, 0, stream>>>(prm); break;
+            case 16: fir2b_kernel<16, 16, true><<<grid, kFir2Threads, 0, stream>>>(prm); break;
+            default: return fail(fe, FENGINE_ERR_INVALID_ARG, "no tiled FIR for %d-bit samples", fe->bits);
+            }
+            return FENGINE_OK;
+        }
         switch (fe->bits) {
         case 4: fir2b_kernel<16, 4><<<grid, kFir2Threads, 0, stream>>>(prm); break;
         case 8: fir2b_kernel<16, 8><<<grid, kFir2Threads, 0, stream>>>(prm); break;
@@ -332,11 +380,17 @@ int launch_fir2(fengine *fe, const Fir2Params &prm, int64_t chunk_len, cudaStrea
         }
         return FENGINE_OK;
     }
+    if (onepol) return fail(fe, FENGINE_ERR_STATE, "no one-pol-layout variant of the 10-bit pol-packed FIR");
     switch (fe->T) {
     case 2: fir2_kernel<2><<<grid, kFir2Threads, 0, stream>>>(prm); break;
     case 4: fir2_kernel<4><<<grid, kFir2Threads, 0, stream>>>(prm); break;
     case 8: fir2_kernel<8><<<grid, kFir2Threads, 0, stream>>>(prm); break;
-    case 16: fir2_kernel<16><<<grid, kFir2Threads, 0, stream>>>(prm); break;
+    case 16:
+        if (fe->l2_persist)
+            FE_CUDA(fe, launch_win(fir2_kernel<16>, grid, dim3(kFir2Threads), 0, stream, &fe->l2_win, prm));
+        else
+            fir2_kernel<16><<<grid, kFir2Threads, 0, stream>>>(prm);
+        break;
     default: return fail(fe, FENGINE_ERR_INVALID_ARG, "no tiled FIR for T=%d", fe->T);
     }
     return FENGINE_OK;
@@ -528,6 +582,15 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
 
     int rc = fused ? FENGINE_OK : ensure_scratch(fe, (size_t)streams * chunk * fe->N);
     if (rc) return rc;
+    if (fe->l2_persist) {
+        int max_win = 0;
+        cudaDeviceGetAttribute(&max_win, cudaDevAttrMaxAccessPolicyWindowSize, fe->device);
+        fe->l2_win.base_ptr = fe->d_scratch;
+        fe->l2_win.num_bytes = std::min<size_t>((size_t)streams * chunk * fe->N * sizeof(float), (size_t)max_win);
+        fe->l2_win.hitRatio = 1.0f;
+        fe->l2_win.hitProp = cudaAccessPropertyPersisting;
+        fe->l2_win.missProp = cudaAccessPropertyStreaming;
+    }
 
     FirParams fp{};
     fp.in = static_cast<const uint8_t *>(in);
@@ -563,8 +626,21 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
     xp.per_spectrum = per_spectrum ? 1 : 0;
 
     const bool packed = use_packed(fe);
+    const bool fir_packed_only = use_packed_fir_onepol_fft(fe);      // pol-packed FIR in front of the one-pol FFT
     Fir2Params fp2{};
     Fft2Params xp2{};
+    if (fir_packed_only) {
+        fp2.in = fp.in;
+        fp2.weights = fp.weights;
+        fp2.g = fp.g;
+        fp2.coarse = fp.coarse;
+        fp2.n_coarse = fp.n_coarse;
+        fp2.stream_bytes = fp.stream_bytes;
+        fp2.rows_in = fp.rows_in;
+        fp2.chunk_cap = chunk;
+        fp2.lgN = fe->lgN;
+        fp2.rows_per_tile = fir_rows_for(fe, m_hi - m_lo, 2 * kFir2Threads, 2);
+    }
     if (packed) {
         fp2.in = fp.in;
         fp2.weights = fp.weights;
@@ -678,10 +754,17 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
             fe->last_launches += 2;
             continue;
         }
-        rc = packed ? launch_fir2(fe, fp2, m1 - m0, stream) : launch_fir(fe, fp, m1 - m0, stream);
+        rc = packed ? launch_fir2(fe, fp2, m1 - m0, stream)
+                    : fir_packed_only ? launch_fir2(fe, fp2, m1 - m0, stream, true) : launch_fir(fe, fp, m1 - m0, stream);
         if (rc) return rc;
         if (fe->profile) FE_CUDA(fe, cudaEventRecord(ev[1], stream));
-        if (packed)
+        if (packed && fe->allow_fft2p && fft2p_supported(fe->n)) {
+            bool &attr = fe->fft2p_attr[out_f32 ? 1 : 0];
+            const int grid = (int)std::min<int64_t>(fe->n_sms, (m1 - m0) * fe->A);
+            cudaError_t ce = fft2p_launch(fe->n, out_f32 != nullptr, xp2, fe->A, grid, !attr, stream);
+            attr = true;
+            if (ce != cudaSuccess) return fail(fe, FENGINE_ERR_CUDA, "persistent FFT launch failed: %s", cudaGetErrorString(ce));
+        } else if (packed)
             rc = out_f32 ? launch_fft2_n<true>(fe, xp2, m1 - m0, stream) : launch_fft2_n<false>(fe, xp2, m1 - m0, stream);
         else
             rc = out_f32 ? launch_fft_n<true>(fe, xp, m1 - m0, stream) : launch_fft_n<false>(fe, xp, m1 - m0, stream);
@@ -1228,7 +1311,7 @@ try {
     const int64_t total = (int64_t)fe->A * fe->P * n_spectra * fe->N;
     if (!use_tiled(fe)) {
         gen_fir_kernel<<<gen_grid(fe, total), 256, 0, s>>>(gen_params(fe, in, n_spectra), g_out);
-    } else if (use_packed(fe)) {
+    } else if (use_packed(fe) || use_packed_fir_onepol_fft(fe)) {
         rc = ensure_scratch(fe, (size_t)total);
         if (rc) return rc;
         Fir2Params fp{};
@@ -1320,6 +1403,16 @@ try {
         fe->allow_fused = value != 0;
         return FENGINE_OK;
     }
+    if (!strcmp(key, "l2_persist")) {                       // value = bytes of L2 set aside for persisting lines (0 = off)
+        if (value < 0) return fail(fe, FENGINE_ERR_INVALID_ARG, "l2_persist < 0");
+        FE_CUDA(fe, cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, (size_t)value));
+        fe->l2_persist = value > 0;
+        return FENGINE_OK;
+    }
+    if (!strcmp(key, "fft_persistent")) {
+        fe->allow_fft2p = value != 0;
+        return FENGINE_OK;
+    }
     if (!strcmp(key, "split")) {
         fe->allow_split = value != 0;
         return FENGINE_OK;
@@ -1397,6 +1490,17 @@ int fengine_debug_pipe_stats(fengine_t *fe, uint64_t *out, int64_t max_words)
     FE_CUDA(fe, cudaMemcpy(out, fe->d_stats, sizeof(uint64_t) * (size_t)words, cudaMemcpyDeviceToHost));
     FE_CUDA(fe, cudaMemset(fe->d_stats, 0, sizeof(unsigned long long) * kStCount * (size_t)fe->n_sms));
     return FENGINE_OK;
+}
+
+int fengine_debug_path(const fengine_t *fe)
+{
+    if (!fe) return -1;
+    if (!use_tiled(fe)) return FENGINE_PATH_GENERIC;
+    if (use_fused(fe)) return FENGINE_PATH_FUSED;
+    if (use_split(fe)) return FENGINE_PATH_SPLIT;
+    if (use_packed(fe)) return FENGINE_PATH_POL_PACKED;
+    if (use_packed_fir_onepol_fft(fe)) return FENGINE_PATH_PACKED_FIR_ONE_POL_FFT;
+    return FENGINE_PATH_ONE_POL;
 }
 
 int fengine_debug_fp32_rate(double *lane_ops_per_second, double *ms_out)

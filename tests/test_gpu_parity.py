@@ -328,6 +328,43 @@ def test_streaming_pushes_equal_one_batch(torch, fb, n, T, A, crange, pushes, eq
     assert diff.max() <= 1 and np.count_nonzero(diff) <= INT8_MISMATCH * diff.size
 
 
+@pytest.mark.parametrize("n,T,bits,S,A", [
+    (32768, 32, 10, 40, 1),         # the paper's tap sweep, Fig. 8 "for 32 768 channels"
+    (32768, 16, 4, 20, 2),          # its bit-depth sweep, Fig. 11
+    (32768, 16, 8, 20, 1),
+    (32768, 16, 12, 20, 1),
+    (32768, 16, 16, 20, 1),
+    (16384, 32, 10, 50, 1),
+    (16384, 16, 12, 37, 2),
+])
+def test_tap_and_bit_depth_sweeps_run_tiled_kernels_at_large_n(torch, fb, n, T, bits, S, A):
+    """SURVEY.md 8(f2) at the survey's size: 32 taps and 4 / 8 / 12 / 16-bit samples at n >= 16384 run a pol-packed FIR
+    (fe_fir3.cuh / fe_fir2b.cuh) that writes the one-pol FFT's scratch layout, not the one-thread-per-output kernels."""
+    sigma = {4: 2.0, 8: 30.0, 10: 32.0, 12: 400.0, 16: 6000.0}[bits]
+    w = si.custom_workload(A=A, n=n, T=T, S=S, P=2, seed=71, coarse_range=(-3 * n, 5 * n), bits=bits, sigma=sigma)
+    w.coarse[:, 1] = w.coarse[:, 0]
+    for a in range(w.A):                                         # the packed stream decodes to the kept samples
+        for p in range(w.P):
+            np.testing.assert_array_equal(oracle.unpack_bits(w.packed[a, p], w.L, bits), w.samples[a, p])
+    fe = make_engine(fb, w, sample_bits=bits) if bits != 10 else make_engine(fb, w)
+    assert fe.path() == "packed_fir_one_pol_fft"
+    got = gpu_run(torch, fe, w)
+    ref = oracle.channelize_f64(w.samples, w.n, w.T, w.weights, coarse=w.coarse, fine_delay=w.fine_delay,
+                                phase=w.phase, gains=w.gains, n_spectra=S)
+    check_parity(got, ref, f"n={n} T={T} bits={bits}")
+    w.coarse[:, 1] += 1                                          # unequal pols: no pol-packed FIR, generic kernels
+    fe.set_coarse_delays(w.coarse)
+    assert fe.path() == "generic"
+
+
+def test_paths_reported_for_the_bench_shapes(fb):
+    for cfg, want in ((1, "one_pol"), (2, "pol_packed"), (3, "one_pol"), (4, "pol_packed")):
+        w = si.make_workload(cfg, n_spectra=4, n_antennas=1)
+        assert make_engine(fb, w).path() == want, cfg
+    w = si.make_workload(2, n_spectra=4, n_antennas=1)
+    assert make_engine(fb, w, split=1).path() == "split" and make_engine(fb, w, fused=1).path() == "fused"
+
+
 def test_fp32_fft_has_no_spurs_with_a_dithered_tone(torch, fb):
     """The paper's precision gate (Fig. 6): a tone in channel 192 of 1024, quantised to 10 bits
     with uniform dither, transformed many times and averaged in double precision.  An FP16 FFT shows harmonics near
