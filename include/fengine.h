@@ -189,12 +189,17 @@ int fengine_debug_fir(fengine_t *fe, const void *in, float *g_out, int64_t n_spe
  * whose FIR -> FFT transposition goes through an L2-resident ring of rows instead of a full-size HBM scratch,
  * fe_pipe.cuh; T = 2, 4, 8, 16; knobs "ring_rows", "fir_warps", "tracks", "segments", "pipe_ctas"), "split" (0/1,
  * default 0, n = 4096: the first radix-16 stage of the transform runs in the FIR kernel and the rest as independent
- * 256-point transforms per warp, fe_split.cuh, the arrangement PAPER.md:403-409 proposes), "host_chunks" (pieces of the fengine_process_host pipeline, 1 = no overlap),
+ * 256-point transforms per warp, fe_split.cuh, the arrangement PAPER.md:403-409 proposes), "fft_persistent" (0/1, default 0: the
+ * pol-packed FFT as one persistent CTA per SM whose rows arrive by bulk copy into the exchange buffer, n <= 4096),
+ * "scratch_fp16" (0/1, default 0; T = 16, n = 1024 or 4096, pol-packed path: the FIR output / FFT input is stored in
+ * FP16 with FP32 arithmetic on both sides, the variant PAPER.md:407 proposes; NOT within the 1e-4 parity bar, it is
+ * the comparison arm of the precision experiment of PAPER.md:149-157), "l2_persist" (bytes of L2 set aside for
+ * persisting lines over the scratch of a chunked call, 0 = off), "host_chunks" (pieces of the fengine_process_host pipeline, 1 = no overlap),
  * "sample_bits" (4, 8, 10 (default), 12, 16: width of the packed input samples, same big-endian bit stream, sample u
  * in bits [b u, b u + b); the stream is then L*b/8 bytes.  The paper's bit-depth sweep.  Widths other
  * than 10 run the tiled kernels on the pol-packed path with 16 taps, else the generic kernels).  Returns INVALID_ARG for
  * unknown keys, and STATE for the options that change the data layout or the path ("sample_bits", "force_generic",
- * "pol_packed", "fused", "split") while a stream is open. */
+ * "pol_packed", "fused", "split", "scratch_fp16") while a stream is open. */
 int fengine_set_option(fengine_t *fe, const char *key, int64_t value);
 
 /*

@@ -14,6 +14,8 @@
 // The one-unit skew per k1 block makes the 128-bit accesses of pass 3 (consecutive lanes = consecutive k1)
 // bank-conflict free.
 #pragma once
+#include <cuda_fp16.h>
+
 #include "fe_common.cuh"
 #include "fe_fft.cuh"
 
@@ -51,6 +53,19 @@ __device__ __forceinline__ cx<f2> unpack_unit_ld(float4 v) { return {f2(v.x, v.y
 struct RowInGlobal {
     const float4 *p;
     __device__ __forceinline__ float4 operator()(int i) const { return ldg_stream_f4(p + i); }
+};
+// FP16 scratch (option "scratch_fp16", the paper's "FP16 for the inputs ... of the FFT, with the internal computations
+// done in FP32"): units of four halves {Re z p0, Re z p1, Im z p0, Im z p1}, 8 bytes
+struct RowInGlobalH16 {
+    const uint2 *p;
+    __device__ __forceinline__ float4 operator()(int i) const
+    {
+        uint2 v;
+        asm volatile("ld.global.cg.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p + i));
+        const float2 a = __half22float2(*reinterpret_cast<const __half2 *>(&v.x));
+        const float2 b = __half22float2(*reinterpret_cast<const __half2 *>(&v.y));
+        return make_float4(a.x, a.y, b.x, b.y);
+    }
 };
 struct RowInShared {
     uint32_t s;                 // shared-space address of unit 0
@@ -415,7 +430,7 @@ constexpr size_t fft2_smem_bytes()
 }
 
 // One CTA per (antenna, spectrum), both pols.
-template <class Plan, bool F32OUT>
+template <class Plan, bool F32OUT, bool H16 = false>
 static __global__ void __launch_bounds__(Plan::tpf, (512 / Plan::tpf) > 0 ? (512 / Plan::tpf) : 1) fft2_kernel(const Fft2Params prm)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -425,8 +440,13 @@ static __global__ void __launch_bounds__(Plan::tpf, (512 / Plan::tpf) > 0 ? (512
     const int a = (int)gridDim.y - 1 - (int)blockIdx.y;
     const int64_t m = prm.m_end - 1 - (int64_t)blockIdx.x;
     if (m < prm.m_begin) return;
-    const RowInGlobal grow{reinterpret_cast<const float4 *>(prm.g + ((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * (int64_t)N * 2)};
-    fft2_row<Plan, F32OUT>(prm, grow, smem_raw, a, m, threadIdx.x, SyncCta{}, [] {});
+    if constexpr (H16) {
+        const RowInGlobalH16 grow{reinterpret_cast<const uint2 *>(prm.g + ((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * (int64_t)N)};
+        fft2_row<Plan, F32OUT>(prm, grow, smem_raw, a, m, threadIdx.x, SyncCta{}, [] {});
+    } else {
+        const RowInGlobal grow{reinterpret_cast<const float4 *>(prm.g + ((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * (int64_t)N * 2)};
+        fft2_row<Plan, F32OUT>(prm, grow, smem_raw, a, m, threadIdx.x, SyncCta{}, [] {});
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------------------

@@ -14,6 +14,8 @@
 // Input staging is the ring of fe_fir.cuh with both pols' 80-byte row segments side by side in a
 // 160-byte slot.  A 5-byte group (4 samples) is shared by the two threads that own its two points.
 #pragma once
+#include <cuda_fp16.h>
+
 #include "fe_common.cuh"
 #include "fe_fir.cuh"
 
@@ -55,6 +57,26 @@ struct Fir2ScratchSink {            // two-kernel path: rows of the linear scrat
     {
         asm volatile("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %5, %6;\n\t@p st.global.v4.f32 [%0], {%1, %2, %3, %4};\n\t}"
                      ::"l"(gp), "f"(cur.x), "f"(cur.y), "f"(cur.z), "f"(cur.w), "r"((unsigned)sp), "r"((unsigned)n_out) : "memory");
+        gp += g_stride;
+        ++sp;
+    }
+};
+
+// FP16 scratch (option "scratch_fp16"): the unit is rounded to four halves and stored as 8 bytes
+struct Fir2ScratchSinkH16 {
+    float *gp;                  // byte address arithmetic in floats: a unit is 2 floats wide, a row N floats
+    size_t g_stride;
+    int sp, n_out;
+    __device__ __forceinline__ void begin_run(int lag, int T, int n_out_) { gp += ((int64_t)lag - T) * (int64_t)g_stride; sp = lag - T; n_out = n_out_; }
+    __device__ __forceinline__ void before_steps(int) {}
+    __device__ __forceinline__ void after_steps(int) {}
+    __device__ __forceinline__ void end_run() {}
+    __device__ __forceinline__ void store(float4 cur)
+    {
+        const __half2 a = __floats2half2_rn(cur.x, cur.y), b = __floats2half2_rn(cur.z, cur.w);
+        asm volatile("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %3, %4;\n\t@p st.global.v2.b32 [%0], {%1, %2};\n\t}"
+                     ::"l"(gp), "r"(*reinterpret_cast<const unsigned int *>(&a)), "r"(*reinterpret_cast<const unsigned int *>(&b)),
+                       "r"((unsigned)sp), "r"((unsigned)n_out) : "memory");
         gp += g_stride;
         ++sp;
     }
@@ -203,7 +225,7 @@ __device__ __forceinline__ void fir2_run(const Fir2Params &prm, const uint8_t *w
     sink.end_run();
 }
 
-template <int T>
+template <int T, bool H16 = false>
 __global__ void __launch_bounds__(kFir2Threads, 4) fir2_kernel(const Fir2Params prm)
 {
     // +16: the second word of the last lane's pol-1 group may lie just past the last slot (never selected)
@@ -226,9 +248,19 @@ __global__ void __launch_bounds__(kFir2Threads, 4) fir2_kernel(const Fir2Params 
             run_end = m + 1;
             while (run_end < m_stop && ctab[run_end] == c) ++run_end;
         }
-        float *grow0 = prm.g + ((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * (int64_t)N * 2;
         const int cr = (int)((int64_t)c & (int64_t)(N - 1));
         const bool mixed = (2 * i_pt + cr < N) && (2 * i_pt + 1 + cr >= N);
+        if constexpr (H16) {
+            float *grow0 = prm.g + ((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * (int64_t)N;
+            Fir2ScratchSinkH16 sink{grow0 + 2 * i_pt, (size_t)N, 0, 0};
+            if (__any_sync(0xffffffffu, mixed))
+                fir2_run<T, true>(prm, wsrc, ring_s, (int64_t)c, m, (int)(run_end - m), i_pt, sink);
+            else
+                fir2_run<T, false>(prm, wsrc, ring_s, (int64_t)c, m, (int)(run_end - m), i_pt, sink);
+            m = run_end;
+            continue;
+        }
+        float *grow0 = prm.g + ((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * (int64_t)N * 2;
         Fir2ScratchSink sink{grow0 + 4 * i_pt, (size_t)N * 2, 0, 0};
         if (__any_sync(0xffffffffu, mixed))
             fir2_run<T, true>(prm, wsrc, ring_s, (int64_t)c, m, (int)(run_end - m), i_pt, sink);

@@ -60,6 +60,8 @@ struct fengine {
     unsigned int *d_ctl = nullptr;
     size_t ctl_words = 0;
     bool allow_fused = false;       // option "fused": the pipelined kernel (fe_pipe.cuh), slower than the two-kernel path today
+    bool scratch_h16 = false;       // option "scratch_fp16": FP16 FIR output / FFT input, not parity grade
+    bool fft_h16_attr[2] = {};
     bool l2_persist = false;        // option "l2_persist": launch the two kernels with a persisting L2 window over the scratch
     cudaAccessPolicyWindow l2_win{};
     bool allow_fft2p = false;       // option "fft_persistent": persistent pol-packed FFT with bulk-copy prefetch (fft2p_kernel); measured slower
@@ -196,6 +198,17 @@ int launch_fft2(fengine *fe, const Fft2Params &prm, int64_t chunk_len, cudaStrea
         attr_set = true;
     }
     dim3 grid((unsigned)chunk_len, (unsigned)fe->A);
+    if constexpr (Plan::n == 1024 || Plan::n == 4096) {
+        if (fe->scratch_h16) {
+            bool &attr16 = fe->fft_h16_attr[F32OUT ? 1 : 0];
+            if (!attr16) {
+                FE_CUDA(fe, cudaFuncSetAttribute(fft2_kernel<Plan, F32OUT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                attr16 = true;
+            }
+            fft2_kernel<Plan, F32OUT, true><<<grid, Plan::tpf, smem, stream>>>(prm);
+            return FENGINE_OK;
+        }
+    }
     if (fe->l2_persist)
         FE_CUDA(fe, launch_win(fft2_kernel<Plan, F32OUT>, grid, dim3(Plan::tpf), smem, stream, &fe->l2_win, prm));
     else
@@ -386,7 +399,9 @@ int launch_fir2(fengine *fe, const Fir2Params &prm, int64_t chunk_len, cudaStrea
     case 4: fir2_kernel<4><<<grid, kFir2Threads, 0, stream>>>(prm); break;
     case 8: fir2_kernel<8><<<grid, kFir2Threads, 0, stream>>>(prm); break;
     case 16:
-        if (fe->l2_persist)
+        if (fe->scratch_h16)
+            fir2_kernel<16, true><<<grid, kFir2Threads, 0, stream>>>(prm);
+        else if (fe->l2_persist)
             FE_CUDA(fe, launch_win(fir2_kernel<16>, grid, dim3(kFir2Threads), 0, stream, &fe->l2_win, prm));
         else
             fir2_kernel<16><<<grid, kFir2Threads, 0, stream>>>(prm);
@@ -577,8 +592,10 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
     if (fe->rg_dirty) return fail(fe, FENGINE_ERR_STATE, "rotation / gain tables are stale (a setter failed)");
 
     const int64_t chunk = fe->chunk_spectra > 0 ? std::min<int64_t>(fe->chunk_spectra, m_hi - m_lo) : m_hi - m_lo;
-    const bool fused = use_fused(fe);
-    const bool split = !fused && use_split(fe);
+    const bool fused = use_fused(fe) && !fe->scratch_h16;
+    const bool split = !fused && use_split(fe) && !fe->scratch_h16;
+    if (fe->scratch_h16 && !(use_packed(fe) && fe->bits == 10))
+        return fail(fe, FENGINE_ERR_STATE, "scratch_fp16 needs the pol-packed path (equal coarse delays in both pols, 10-bit samples)");
 
     int rc = fused ? FENGINE_OK : ensure_scratch(fe, (size_t)streams * chunk * fe->N);
     if (rc) return rc;
@@ -758,7 +775,7 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
                     : fir_packed_only ? launch_fir2(fe, fp2, m1 - m0, stream, true) : launch_fir(fe, fp, m1 - m0, stream);
         if (rc) return rc;
         if (fe->profile) FE_CUDA(fe, cudaEventRecord(ev[1], stream));
-        if (packed && fe->allow_fft2p && fft2p_supported(fe->n)) {
+        if (packed && fe->allow_fft2p && fft2p_supported(fe->n) && !fe->scratch_h16) {
             bool &attr = fe->fft2p_attr[out_f32 ? 1 : 0];
             const int grid = (int)std::min<int64_t>(fe->n_sms, (m1 - m0) * fe->A);
             cudaError_t ce = fft2p_launch(fe->n, out_f32 != nullptr, xp2, fe->A, grid, !attr, stream);
@@ -1307,6 +1324,7 @@ try {
     int rc = check_call(fe, in, g_out, n_spectra);
     if (rc || n_spectra == 0) return rc;
     if (fe->stream_off != 0) return fail(fe, FENGINE_ERR_STATE, "a stream is open: the debug hooks see the shifted delay table");
+    if (fe->scratch_h16) return fail(fe, FENGINE_ERR_STATE, "fengine_debug_fir shows the FP32 FIR output: switch scratch_fp16 off");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const int64_t total = (int64_t)fe->A * fe->P * n_spectra * fe->N;
     if (!use_tiled(fe)) {
@@ -1368,7 +1386,7 @@ try {
     if (!fe || !key) return FENGINE_ERR_INVALID_ARG;
     fe->err.clear();
     if (fe->stream_off != 0 && (!strcmp(key, "sample_bits") || !strcmp(key, "force_generic") || !strcmp(key, "pol_packed") ||
-                                !strcmp(key, "fused") || !strcmp(key, "split")))
+                                !strcmp(key, "fused") || !strcmp(key, "split") || !strcmp(key, "scratch_fp16")))
         return fail(fe, FENGINE_ERR_STATE, "option %s changes the data layout or the path and cannot change while a stream is open", key);
     if (!strcmp(key, "chunk_spectra")) {
         if (value < 0) return fail(fe, FENGINE_ERR_INVALID_ARG, "chunk_spectra < 0");
@@ -1401,6 +1419,12 @@ try {
     }
     if (!strcmp(key, "fused")) {
         fe->allow_fused = value != 0;
+        return FENGINE_OK;
+    }
+    if (!strcmp(key, "scratch_fp16")) {
+        if (value && !(fe->T == 16 && (fe->n == 1024 || fe->n == 4096) && fe->P == 2))
+            return fail(fe, FENGINE_ERR_INVALID_ARG, "scratch_fp16 exists for the pol-packed path with T = 16 and n = 1024 or 4096");
+        fe->scratch_h16 = value != 0;
         return FENGINE_OK;
     }
     if (!strcmp(key, "l2_persist")) {                       // value = bytes of L2 set aside for persisting lines (0 = off)
