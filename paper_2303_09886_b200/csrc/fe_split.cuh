@@ -40,7 +40,8 @@ constexpr int kStagePitch = 258;                    // words per ka row of the s
 struct SplitParams {
     Fir2Params fir;           // in, weights, g (= y), coarse, n_coarse, stream_bytes, rows_in, m_begin, m_end, chunk_cap, lgN, rows_per_tile
     Fft2Params fft;           // g (= y), out, out_f32, tpost, rg2, coarse, fine_d, fine_phi, n_coarse, n_fine, m_begin, m_end, chunk_cap, n_spectra, per_spectrum
-    const float2 *tw1;        // [K1][256]  W_n^{ka i'}     (cos, -sin)
+    const float2 *tw1;        // [K1][M]    W_n^{ka i'}     (cos, -sin); M = n / K1 points per stage-2 transform
+    const float2 *ptw1, *ptw2;  // M > 256: pass twiddles of the M-point plan of the pair kernel (fe_fft2.cuh layout)
     const float2 *tw256;      // [16][16]   W_256^{kb t}
 };
 
@@ -72,7 +73,7 @@ __device__ __forceinline__ void sts_f4(uint32_t saddr, float4 v)
 //     so that step s finishes row s - T of the run on every lane and the row goes to tile slot s mod 16.
 // Blocks of eight steps are handed to the butterfly warps through full / empty mbarriers; gx counts the blocks of
 // this CTA since its start (buffer gx & 1, phase gx >> 1).
-template <int T, int IL>
+template <int T, int IL, int M>
 __device__ __forceinline__ void split_fir_run(const Fir2Params &prm, const uint8_t *abase, int i0, int fw, uint32_t ring_s,
                                               int64_t c, int64_t m0, int n_out, uint32_t tile_thr, uint32_t full0,
                                               uint32_t empty0, unsigned &gx)
@@ -85,7 +86,7 @@ __device__ __forceinline__ void split_fir_run(const Fir2Params &prm, const uint8
     const int N = 1 << prm.lgN;
     const int lane = threadIdx.x & 31;
     const int pt = 32 * fw + lane;                              // point of the CTA: q = pt / IL, il = pt % IL
-    const int i_pt = i0 + (pt % IL) + kSubM * (pt / IL);
+    const int i_pt = i0 + (pt % IL) + M * (pt / IL);
     const int cr = (int)(c & (int64_t)(N - 1));
     const int64_t cq = (c - cr) >> prm.lgN;
     const int v0 = 2 * i_pt;
@@ -133,7 +134,7 @@ __device__ __forceinline__ void split_fir_run(const Fir2Params &prm, const uint8
         const int pol = rem / (5 * NP), k = rem - pol * (5 * NP);
         const int piece = k / 5, kk = k - piece * 5;
         const int p0 = 32 * fw + piece * (32 / NP);
-        const int ip = i0 + (p0 % IL) + kSubM * (p0 / IL);      // first point of the piece: a multiple of 32 / NP
+        const int ip = i0 + (p0 % IL) + M * (p0 / IL);      // first point of the piece: a multiple of 32 / NP
         dst[t] = ring_s + (uint32_t)(row * kFir2SlotBytes + pol * kFir2SegBytes + k * CB);
         src[t] = abase + pol * prm.stream_bytes + (R0 + row) * (int64_t)row_bytes + (ip / 2) * 5 + kk * CB;
         trow[t] = has ? row - q_lo : -0x40000000;
@@ -224,12 +225,12 @@ __device__ __forceinline__ void split_fir_run(const Fir2Params &prm, const uint8
 // K1 = 16: thread (r = bt / 16, il = bt % 16) of the 128 butterfly threads takes row r of a block and the sixteen
 // points il + 16 q of the tile, and writes y[ka][i0 + il], ka < 16.  The twiddles W_n^{(i0 + il) ka} belong to the
 // thread for the whole kernel (registers).
-template <int T, int K1>
+template <int T, int K1, int M>
 __device__ __forceinline__ void split_bf_run(const Fir2Params &prm, int a, int i0, int bt, uint32_t tile_s, int64_t m0,
                                              int n_out, const float2 (&tw)[K1], uint32_t full0, uint32_t empty0, unsigned &gx)
 {
     static_assert(K1 == 16, "stage-1 radix 16");
-    constexpr int IL = kSubM / K1;
+    constexpr int IL = 256 / K1;
     const int lane = threadIdx.x & 31;
     const int il = bt % IL, r = bt / IL;
     const int n_blocks = (n_out + T + kFirUnroll - 1) / kFirUnroll * (kFirUnroll / 8);
@@ -249,12 +250,12 @@ __device__ __forceinline__ void split_bf_run(const Fir2Params &prm, int a, int i
         if (valid) {
             Dif<K1, f2>::run(v);
             float4 *yp = reinterpret_cast<float4 *>(prm.g) +
-                         (((int64_t)a * prm.chunk_cap + (m0 + rho - prm.m_begin)) * K1) * kSubM + i0 + il;
+                         (((int64_t)a * prm.chunk_cap + (m0 + rho - prm.m_begin)) * K1) * M + i0 + il;
 #pragma unroll
             for (int ka = 0; ka < K1; ++ka) {
                 cx<f2> y = v[ka];
                 if (ka > 0) y = cmul(v[ka], tw[ka].x, tw[ka].y);
-                stg_stream_f4(yp + ka * kSubM, pack_unit(y));
+                stg_stream_f4(yp + ka * M, pack_unit(y));
             }
         }
     }
@@ -266,11 +267,11 @@ constexpr size_t split_producer_smem() { return (size_t)kSplitTileBytes + kSplit
 #ifndef FE_SPLIT_LB
 #define FE_SPLIT_LB kSplitProducerThreads
 #endif
-template <int T, int K1>
+template <int T, int K1, int M = kSubM>
 __global__ void __launch_bounds__(FE_SPLIT_LB, 1) split_fir_kernel(const __grid_constant__ SplitParams prm)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    constexpr int IL = kSubM / K1;
+    constexpr int IL = 256 / K1;                                 // consecutive i' per q: the CTA holds 256 points
     const int tid = threadIdx.x, warp = tid >> 5;
     const uint32_t s_base = smem_u32(smem_raw);
     const uint32_t tile_s = s_base;
@@ -307,7 +308,7 @@ __global__ void __launch_bounds__(FE_SPLIT_LB, 1) split_fir_kernel(const __grid_
         for (int64_t m = m_first; m < m_stop;) {
             int32_t c;
             const int64_t run_end = next_run(m, c);
-            split_fir_run<T, IL>(prm.fir, abase, i0, warp, ring_s, (int64_t)c, m, (int)(run_end - m), tile_s + (uint32_t)tid * 16u,
+            split_fir_run<T, IL, M>(prm.fir, abase, i0, warp, ring_s, (int64_t)c, m, (int)(run_end - m), tile_s + (uint32_t)tid * 16u,
                                  full0, empty0, gx);
             m = run_end;
         }
@@ -315,11 +316,11 @@ __global__ void __launch_bounds__(FE_SPLIT_LB, 1) split_fir_kernel(const __grid_
         const int bt = tid - 32 * kSplitFirWarps;
         float2 tw[K1];
 #pragma unroll
-        for (int ka = 0; ka < K1; ++ka) tw[ka] = __ldg(prm.tw1 + ka * kSubM + i0 + bt % IL);
+        for (int ka = 0; ka < K1; ++ka) tw[ka] = __ldg(prm.tw1 + ka * M + i0 + bt % IL);
         for (int64_t m = m_first; m < m_stop;) {
             int32_t c;
             const int64_t run_end = next_run(m, c);
-            split_bf_run<T, K1>(prm.fir, a, i0, bt, tile_s, m, (int)(run_end - m), tw, full0, empty0, gx);
+            split_bf_run<T, K1, M>(prm.fir, a, i0, bt, tile_s, m, (int)(run_end - m), tw, full0, empty0, gx);
             m = run_end;
         }
     }
@@ -539,9 +540,166 @@ __global__ void __launch_bounds__(SplitFftSmem<K1>::warps * 32, 2) split_fft_ker
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// consumer for n >= 16384: stage 2 is K1 = 16 transforms of M = n / 16 = 1024 or 2048 points, too large for a warp.
+// One CTA = two teams of Plan::tpf threads, one team per transform of the mirror pair (ka, K1 - ka); each team runs
+// passes 1 and 2 of the pol-packed M-point plan of fe_fft2.cuh in its own exchange buffer, and the last pass takes
+// the mirror halves out of the OTHER team's buffer (pair 0: ka = 0 and K1 / 2 mirror onto themselves).  This replaces
+// the pol-sequential four-pass transform of fe_fft.cuh, which needs two sweeps over the row at n = 32768 because the
+// whole row does not fit one SM's shared memory (BASELINE.json north_star (b): "a four-step decomposition through
+// HBM ... for n = 32768").  A transform ka holds the channels k = ka (mod 16), so a thread's output words are 64
+// bytes apart; the eight CTAs of a spectrum run side by side and their words meet in L2.
+// ---------------------------------------------------------------------------------------------------------------
+struct SplitPhaseBig {       // per (CTA, spectrum), per-spectrum delay mode only; units {re p0, re p1, im p0, im p1}
+    float4 ea[2];            // [team]: exp(i phi) exp(-2 pi i d_eff ka / N)
+    float4 elo[16];          // exp(-2 pi i d_eff K1 K_lo / N)
+    float4 ehi[16];          // exp(-2 pi i d_eff K1 16 K_hi / N)
+    float4 step[9];          // exp(-2 pi i d_eff K1 Q kq / N), kq <= R3 / 2
+    float4 c3;               // exp(2 i phi) exp(-i pi d_eff)
+};
+
+template <class Plan, int K1>
+__device__ __forceinline__ void split_big_setup_phase(const Fft2Params &prm, SplitPhaseBig *sph, int a, int64_t m, int pair,
+                                                      int p, int lane)
+{
+    constexpr int N = 2 * K1 * Plan::n, Q = Plan::Q, H = Plan::R3 / 2;
+    const int64_t st = (int64_t)a * 2 + p;
+    const int32_t c = prm.coarse[st * prm.n_coarse + (prm.n_coarse == 1 ? 0 : m)];
+    const int cr = (int)(c & (N - 1));
+    const double d = (double)prm.fine_d[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
+    const double phi = (double)prm.fine_phi[st * prm.n_fine + (prm.n_fine == 1 ? 0 : m)];
+    auto phasor = [&](int k) { return phasor_turns(-(d / (double)N) * (double)k - (double)(((int64_t)cr * k) & (N - 1)) / (double)N); };
+    auto put = [&](float4 *dst4, float2 v) {
+        float *dst = reinterpret_cast<float *>(dst4);
+        dst[p] = v.x;
+        dst[2 + p] = v.y;
+    };
+    double sphi, cphi;
+    sincos(phi, &sphi, &cphi);
+    const float2 ephi = make_float2((float)cphi, (float)sphi);
+    if (lane < 2) put(&sph->ea[lane], cmulf(phasor(pair == 0 ? (lane ? K1 / 2 : 0) : (lane ? K1 - pair : pair)), ephi));
+    if (lane < 16) put(&sph->elo[lane], phasor(K1 * lane));
+    if (lane >= 16 && lane < 16 + Q / 16) put(&sph->ehi[lane - 16], phasor(K1 * 16 * (lane - 16)));
+    if (lane < H + 1) put(&sph->step[lane], phasor(K1 * Q * lane));
+    if (lane == 31) {
+        double s, c_;
+        sincos(2.0 * phi, &s, &c_);
+        const float2 e2 = make_float2((float)c_, (float)s);
+        float2 h = phasor_turns(-0.5 * d);
+        if (cr & 1) { h.x = -h.x; h.y = -h.y; }
+        put(&sph->c3, cmulf(e2, h));
+    }
+}
+
+template <class Plan>
+struct SplitBigSmem {
+    static constexpr uint32_t buf_bytes = ((uint32_t)Plan::units * 16u + 127u) & ~127u;
+    static constexpr uint32_t phase_off = 2 * buf_bytes;
+    static constexpr size_t bytes = phase_off + sizeof(SplitPhaseBig);
+};
+
+// grid (K1 / 2 pairs, spectra of the chunk, antennas); 2 * Plan::tpf threads
+template <class Plan, int K1, bool F32OUT>
+__global__ void __launch_bounds__(2 * Plan::tpf, 512 / (2 * Plan::tpf)) split_pair_kernel(const __grid_constant__ SplitParams sp)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    using SM = SplitBigSmem<Plan>;
+    constexpr int M = Plan::n, n = K1 * M, R = Plan::R3, H = R / 2, Q = Plan::Q, tpf = Plan::tpf;
+    static_assert(Plan::SW == 1 && Q == tpf, "one-sweep plan, one residue per thread");
+    const Fft2Params &prm = sp.fft;
+    const int team = threadIdx.x / tpf, K = threadIdx.x - team * tpf;
+    const int pair = blockIdx.x;
+    const int a = blockIdx.z;
+    const int64_t m = prm.m_begin + blockIdx.y;
+    const int ka = pair == 0 ? (team ? K1 / 2 : 0) : (team ? K1 - pair : pair);
+    float4 *sm = reinterpret_cast<float4 *>(smem_raw + (size_t)team * SM::buf_bytes);
+    const float4 *other = reinterpret_cast<const float4 *>(smem_raw + (size_t)(pair == 0 ? team : 1 - team) * SM::buf_bytes);
+    SplitPhaseBig *sph = reinterpret_cast<SplitPhaseBig *>(smem_raw + SM::phase_off);
+    if (prm.per_spectrum && threadIdx.x < 64) split_big_setup_phase<Plan, K1>(prm, sph, a, m, pair, threadIdx.x >> 5, threadIdx.x & 31);
+
+    // passes 1 and 2 of the M-point transform of y[ka][.] (pass twiddles of the M-point plan)
+    const RowInGlobal yrow{reinterpret_cast<const float4 *>(prm.g) + (((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * K1 + ka) * (int64_t)M};
+    fft2_pass1<Plan>(yrow, sm, sp.ptw1, K);
+    __syncthreads();
+    fft2_pass2<Plan>(sm, sp.ptw2, K);
+    __syncthreads();
+
+    // last pass: residue K of this transform, Z[ka + K1 (K + Q kq)]
+    const bool self0 = pair == 0 && team == 0;                 // ka = 0 mirrors onto itself with the index shifted by one
+    const bool special = self0 && K == 0;
+    float4 *mine = sm + (K & (Plan::R1 - 1)) * Plan::blk + (K / Plan::R1) * Plan::M2;
+    const int Kp = self0 ? (Q - K) & (Q - 1) : Q - 1 - K;
+    const float4 *theirs = other + (Kp & (Plan::R1 - 1)) * Plan::blk + (Kp / Plan::R1) * Plan::M2;
+    cx<f2> z[R];
+#pragma unroll
+    for (int t = 0; t < R; ++t) z[t] = unpack_unit(mine[t]);
+    Dif<R, f2>::run(z);
+    if (special) {
+#pragma unroll
+        for (int j = 0; j < H; ++j) mine[j] = pack_unit(z[(R - j) % R]);
+        mine[H] = pack_unit(z[H]);
+    } else {
+#pragma unroll
+        for (int j = 0; j < H; ++j) mine[j] = pack_unit(z[R - 1 - j]);
+    }
+
+    const int k0 = ka + K1 * K;
+    const float2 tpK = __ldg(prm.tpost + k0);
+    const float4 *__restrict__ gtab = reinterpret_cast<const float4 *>(prm.rg2) + (int64_t)a * n;
+    uint32_t *rec = F32OUT ? nullptr : reinterpret_cast<uint32_t *>(prm.out + (((int64_t)a * prm.n_spectra + m) * n) * 4);
+    float4 *yout = F32OUT ? reinterpret_cast<float4 *>(prm.out_f32 + (((int64_t)a * prm.n_spectra + m) * n) * 4) : nullptr;
+    float4 gA[H], gB[H];
+#pragma unroll
+    for (int kq = 0; kq < H; ++kq) {
+        const int kA = k0 + K1 * Q * kq;
+        gA[kq] = ldg_keep_f4(gtab + kA);
+        gB[kq] = ldg_keep_f4(gtab + ((n - kA) & (n - 1)));
+    }
+    __syncthreads();                                           // upper halves are in the exchange buffers
+    cx<f2> base = {f2(1.f, 1.f), f2(0.f, 0.f)};
+    if (prm.per_spectrum)
+        base = cmul2(cmul2(unpack_unit(sph->ea[team]), unpack_unit(sph->elo[K & 15])), unpack_unit(sph->ehi[K >> 4]));
+    auto rot_gain = [&](int kq, cx<f2> gA_, cx<f2> gB_, cx<f2> &rgA, cx<f2> &rgB) {
+        if (prm.per_spectrum) {
+            const cx<f2> E = cmul2(base, unpack_unit(sph->step[kq]));
+            const cx<f2> Ec = {E.re, -E.im};
+            const cx<f2> eA = {E.re * 0.5f, E.im * 0.5f};
+            const cx<f2> eB0 = cmul2(unpack_unit(sph->c3), Ec);
+            const cx<f2> eB = {eB0.re * 0.5f, eB0.im * 0.5f};
+            rgA = cmul2(eA, gA_);
+            rgB = cmul2(eB, gB_);
+        } else {
+            rgA = gA_;
+            rgB = gB_;
+        }
+    };
+#pragma unroll
+    for (int kq = 0; kq < H; ++kq) {
+        const int kA = k0 + K1 * Q * kq, kB = n - kA;
+        const cx<f2> zm = unpack_unit(theirs[kq]);
+        cx<f2> rgA, rgB;
+        rot_gain(kq, unpack_unit(gA[kq]), unpack_unit(gB[kq]), rgA, rgB);
+        float2 tp = tpK;
+        if (kq > 0) {                                          // (sin, cos)(2 pi kA / N): rotate the thread's word by 2 pi kq / (2 R)
+            constexpr int st = 16 / R;
+            const float cphi = w32_cos(kq * st), sphi = w32_sin(kq * st);
+            tp = make_float2(fmaf(tpK.x, cphi, tpK.y * sphi), fmaf(-tpK.x, sphi, tpK.y * cphi));
+        }
+        fft2_epilogue<F32OUT>(z[kq], zm, tp, rgA, rgB, kA, kB, n, rec, yout);
+    }
+    if (special) {                                             // channel n/2 mirrors onto itself
+        const cx<f2> zh = unpack_unit(mine[H]);
+        cx<f2> rgA, rgB;
+        const cx<f2> gh = unpack_unit(__ldg(gtab + n / 2));
+        rot_gain(H, gh, gh, rgA, rgB);
+        fft2_epilogue<F32OUT>(zh, zh, make_float2(1.0f, 0.0f), rgA, rgB, n / 2, n, n, rec, yout);
+    }
+}
+
 // launchers (fe_split.cu)
 cudaError_t split_launch_fir(int T, int n, const SplitParams &prm, dim3 grid, bool set_attr, cudaStream_t stream);
 cudaError_t split_launch_fft(int n, bool f32out, const SplitParams &prm, dim3 grid, bool set_attr, cudaStream_t stream);
 bool split_supported(int n, int T);
+bool split_is_big(int n);
 
 }  // namespace fe

@@ -66,8 +66,9 @@ struct fengine {
     cudaAccessPolicyWindow l2_win{};
     bool allow_fft2p = false;       // option "fft_persistent": persistent pol-packed FFT with bulk-copy prefetch (fft2p_kernel); measured slower
     bool fft2p_attr[2] = {};
-    bool allow_split = false;       // option "split": FIR + first transform stage / 256-point transforms per warp (fe_split.cuh); measured slower
+    int opt_split = -1;             // option "split" (fe_split.cuh): -1 = where it wins (n >= 16384), 0 = never, 1 = wherever it exists
     float2 *d_sp_tw1 = nullptr, *d_sp_tw256 = nullptr;   // its twiddle tables
+    float2 *d_sp_ptw1 = nullptr, *d_sp_ptw2 = nullptr;   // n >= 16384: pass twiddles of the n/16-point plan of the pair kernel
     bool split_attr[3] = {};        // shared-memory attribute set (producer, consumer int8, consumer f32)
     int ring_rows = 32;             // option "ring_rows" (D: rows per track, a power of two >= 16)
     int opt_fir_warps = 0;          // option "fir_warps" (FIR warps per CTA, 0 = as many as the block allows)
@@ -250,7 +251,9 @@ bool use_fused(const fengine *fe)
 
 bool use_split(const fengine *fe)
 {
-    return use_packed(fe) && fe->allow_split && fe->bits == 10 && fe->d_sp_tw1 && split_supported(fe->n, fe->T);
+    if (!fe->tiled || !fe->d_sp_tw1 || fe->P != 2 || !fe->pols_equal || !fe->allow_packed || fe->bits != 10) return false;
+    if (!split_supported(fe->n, fe->T) || fe->opt_split == 0) return false;
+    return fe->opt_split == 1 || split_is_big(fe->n);
 }
 
 // Rows per producer tile of the split path: one CTA per SM, so the tile count is chosen for whole waves over the SMs
@@ -658,7 +661,7 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
         fp2.lgN = fe->lgN;
         fp2.rows_per_tile = fir_rows_for(fe, m_hi - m_lo, 2 * kFir2Threads, 2);
     }
-    if (packed) {
+    if (packed || split) {
         fp2.in = fp.in;
         fp2.weights = fp.weights;
         fp2.g = fp.g;
@@ -758,13 +761,16 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
             sp.fir.rows_per_tile = split_rows_for(fe, m1 - m0);
             sp.tw1 = fe->d_sp_tw1;
             sp.tw256 = fe->d_sp_tw256;
+            sp.ptw1 = fe->d_sp_ptw1;
+            sp.ptw2 = fe->d_sp_ptw2;
             const dim3 gridp((unsigned)(fe->n / kSubM), (unsigned)((m1 - m0 + sp.fir.rows_per_tile - 1) / sp.fir.rows_per_tile), (unsigned)fe->A);
             cudaError_t ce = split_launch_fir(fe->T, fe->n, sp, gridp, !fe->split_attr[0], stream);
             fe->split_attr[0] = true;
             if (ce != cudaSuccess) return fail(fe, FENGINE_ERR_CUDA, "split producer launch failed: %s", cudaGetErrorString(ce));
             if (fe->profile) FE_CUDA(fe, cudaEventRecord(ev[1], stream));
             bool &attr = fe->split_attr[out_f32 ? 2 : 1];
-            ce = split_launch_fft(fe->n, out_f32 != nullptr, sp, dim3((unsigned)(m1 - m0), (unsigned)fe->A), !attr, stream);
+            const dim3 gridc = split_is_big(fe->n) ? dim3(8u, (unsigned)(m1 - m0), (unsigned)fe->A) : dim3((unsigned)(m1 - m0), (unsigned)fe->A);
+            ce = split_launch_fft(fe->n, out_f32 != nullptr, sp, gridc, !attr, stream);
             attr = true;
             if (ce != cudaSuccess) return fail(fe, FENGINE_ERR_CUDA, "split consumer launch failed: %s", cudaGetErrorString(ce));
             if (fe->profile) FE_CUDA(fe, cudaEventRecord(ev[2], stream));
@@ -860,16 +866,28 @@ try {
             case 8192: rc = build_tables2<Plan2_8192>(fe); break;
             }
         }
-        if (rc == FENGINE_OK && fe->packed_ok && split_supported(fe->n, fe->T)) {
-            const int K1 = fe->n / kSubM;
-            if (cudaMalloc(&fe->d_sp_tw1, sizeof(float2) * (size_t)K1 * kSubM) == cudaSuccess &&
-                cudaMalloc(&fe->d_sp_tw256, sizeof(float2) * 256) == cudaSuccess) {
-                build_scalar_twiddles<<<(K1 * kSubM + 255) / 256, 256>>>(fe->d_sp_tw1, K1, kSubM, fe->n);
+        if (rc == FENGINE_OK && fe->P == 2 && split_supported(fe->n, fe->T)) {
+            const int K1 = 16, M = fe->n / K1;
+            bool okm = cudaMalloc(&fe->d_sp_tw1, sizeof(float2) * (size_t)K1 * M) == cudaSuccess &&
+                       cudaMalloc(&fe->d_sp_tw256, sizeof(float2) * 256) == cudaSuccess;
+            if (okm && !fe->d_rg2) okm = cudaMalloc(&fe->d_rg2, sizeof(float4) * (size_t)fe->A * fe->n) == cudaSuccess;
+            if (okm) {
+                build_scalar_twiddles<<<(K1 * M + 255) / 256, 256>>>(fe->d_sp_tw1, K1, M, fe->n);
                 build_scalar_twiddles<<<1, 256>>>(fe->d_sp_tw256, 16, 16, 256);
-                if (cudaGetLastError() != cudaSuccess) rc = FENGINE_ERR_CUDA;
-            } else {
-                rc = FENGINE_ERR_ALLOC;
             }
+            if (okm && split_is_big(fe->n)) {                 // the M-point plan of the pair kernel: Plan2_1024 / Plan2_2048
+                const int M1 = M / 16, R2 = 8, M2 = M1 / R2;
+                okm = cudaMalloc(&fe->d_sp_ptw1, sizeof(float2) * 16 * (size_t)M1) == cudaSuccess &&
+                      cudaMalloc(&fe->d_sp_ptw2, sizeof(float2) * (size_t)R2 * M2) == cudaSuccess;
+                if (okm) {
+                    build_scalar_twiddles<<<(16 * M1 + 255) / 256, 256>>>(fe->d_sp_ptw1, 16, M1, M);
+                    build_scalar_twiddles<<<(R2 * M2 + 255) / 256, 256>>>(fe->d_sp_ptw2, R2, M2, M1);
+                }
+            }
+            if (!okm)
+                rc = FENGINE_ERR_ALLOC;
+            else if (cudaGetLastError() != cudaSuccess)
+                rc = FENGINE_ERR_CUDA;
         }
         ok = rc == FENGINE_OK;
     }
@@ -909,6 +927,8 @@ void fengine_destroy(fengine_t *fe)
     cudaFree(fe->d_rg2);
     cudaFree(fe->d_sp_tw1);
     cudaFree(fe->d_sp_tw256);
+    cudaFree(fe->d_sp_ptw1);
+    cudaFree(fe->d_sp_ptw2);
     cudaFree(fe->d_scratch);
     cudaFree(fe->d_ring);
     cudaFree(fe->d_ctl);
@@ -1438,7 +1458,8 @@ try {
         return FENGINE_OK;
     }
     if (!strcmp(key, "split")) {
-        fe->allow_split = value != 0;
+        if (value < -1 || value > 1) return fail(fe, FENGINE_ERR_INVALID_ARG, "split must be -1 (auto), 0 or 1");
+        fe->opt_split = (int)value;
         return FENGINE_OK;
     }
     if (!strcmp(key, "ring_rows")) {

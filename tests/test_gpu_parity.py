@@ -358,11 +358,13 @@ def test_tap_and_bit_depth_sweeps_run_tiled_kernels_at_large_n(torch, fb, n, T, 
 
 
 def test_paths_reported_for_the_bench_shapes(fb):
-    for cfg, want in ((1, "one_pol"), (2, "pol_packed"), (3, "one_pol"), (4, "pol_packed")):
+    for cfg, want in ((1, "one_pol"), (2, "pol_packed"), (3, "split"), (4, "pol_packed")):
         w = si.make_workload(cfg, n_spectra=4, n_antennas=1)
         assert make_engine(fb, w).path() == want, cfg
     w = si.make_workload(2, n_spectra=4, n_antennas=1)
     assert make_engine(fb, w, split=1).path() == "split" and make_engine(fb, w, fused=1).path() == "fused"
+    w = si.make_workload(3, n_spectra=4, n_antennas=1)
+    assert make_engine(fb, w, split=0).path() == "one_pol"
 
 
 def test_fp32_fft_has_no_spurs_with_a_dithered_tone(torch, fb):
@@ -515,24 +517,29 @@ def test_fused_kernel_matches_oracle_and_two_kernel_path(torch, fb, n, T, S, A, 
     np.testing.assert_array_equal(fused["out"], plain["out"])          # same arithmetic, same order: identical bytes
 
 
-@pytest.mark.parametrize("T,S,A,per_spectrum,opts", [
-    (16, 150, 2, False, dict()),
-    (16, 333, 1, False, dict(fir_rows=40)),                             # several row tiles, ragged last one
-    (16, 3, 1, False, dict()),                                          # fewer rows than one block of eight
-    (8, 70, 2, True, dict()),                                           # per-spectrum delays: a run per coarse delay
-    (4, 45, 3, False, dict(chunk_spectra=16)),
-    (2, 40, 1, False, dict()),
+@pytest.mark.parametrize("n,T,S,A,per_spectrum,opts", [
+    (4096, 16, 150, 2, False, dict()),
+    (4096, 16, 333, 1, False, dict(fir_rows=40)),                       # several row tiles, ragged last one
+    (4096, 16, 3, 1, False, dict()),                                    # fewer rows than one block of eight
+    (4096, 8, 70, 2, True, dict()),                                     # per-spectrum delays: a run per coarse delay
+    (4096, 4, 45, 3, False, dict(chunk_spectra=16)),
+    (4096, 2, 40, 1, False, dict()),
+    (32768, 16, 40, 2, False, dict()),                                  # n >= 16384: pairs of n/16-point transforms per CTA
+    (32768, 8, 23, 1, True, dict()),
+    (16384, 16, 61, 1, False, dict(fir_rows=20)),
+    (16384, 4, 30, 2, True, dict(chunk_spectra=16)),
 ])
-def test_split_path_matches_oracle(torch, fb, T, S, A, per_spectrum, opts):
+def test_split_path_matches_oracle(torch, fb, n, T, S, A, per_spectrum, opts):
     """Option split (fe_split.cuh): the first radix-16 stage of the transform runs with the FIR,
-    the rest as independent 256-point transforms per warp; n = 4096."""
-    w = si.custom_workload(A=A, n=4096, T=T, S=S, P=2, seed=37, per_spectrum=per_spectrum, coarse_range=(-5000, 3 * 4096))
+    the rest as independent n/16-point transforms (per warp at n = 4096, per pair of teams at n >= 16384)."""
+    w = si.custom_workload(A=A, n=n, T=T, S=S, P=2, seed=37, per_spectrum=per_spectrum, coarse_range=(-5000, 3 * n))
     w.coarse[:, 1] = w.coarse[:, 0]
     ref = oracle_run(w)
     fe = make_engine(fb, w, split=1, **opts)
+    assert fe.path() == "split"
     got = gpu_run(torch, fe, w)
     assert fe.last_launch_count() == 2 * (1 if "chunk_spectra" not in opts else -(-S // opts["chunk_spectra"]))
-    check_parity(got, ref, f"split T={T} S={S} A={A}")
+    check_parity(got, ref, f"split n={n} T={T} S={S} A={A}")
 
 
 def test_layout_options_and_debug_hooks_are_refused_while_a_stream_is_open(torch, fb):
