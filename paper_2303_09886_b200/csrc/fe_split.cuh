@@ -329,6 +329,20 @@ __global__ void __launch_bounds__(FE_SPLIT_LB, 1) split_fir_kernel(const __grid_
 // ---------------------------------------------------------------------------------------------------------------
 // consumer: stage 2 of the transform and the epilogue
 // ---------------------------------------------------------------------------------------------------------------
+// The consumers read the gain (x rotation) table in "split order", entry (k mod K1) * M + k / K1 for channel k: the
+// threads of a transform ka hold the channels ka + K1 k' with consecutive k', which natural order would spread over one
+// 128-byte line per lane.
+template <int K1, int M>
+__device__ __forceinline__ int split_gidx(int k) { return (k & (K1 - 1)) * M + k / K1; }
+
+static __global__ void permute_rg2_split(float4 *dst, const float4 *src, int n, int K1, int A)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int a = blockIdx.y;
+    if (k >= n || a >= A) return;
+    dst[(int64_t)a * n + (k % K1) * (n / K1) + k / K1] = src[(int64_t)a * n + k];
+}
+
 struct SplitPhase {          // per spectrum, per-spectrum delay mode only; units {re p0, re p1, im p0, im p1}
     float4 ea[32];           // exp(i phi) exp(-2 pi i d_eff ka / N), ka < K1
     float4 et[16];           // exp(-2 pi i d_eff K1 t / N)
@@ -463,8 +477,8 @@ __device__ __forceinline__ void split_sub256_pair(const Fft2Params &prm, const f
 #pragma unroll
     for (int kq = 0; kq < 8; ++kq) {
         const int kA = k0 + 16 * K1 * kq;
-        gA[kq] = ldg_keep_f4(gtab + kA);
-        gB[kq] = ldg_keep_f4(gtab + ((n - kA) & (n - 1)));
+        gA[kq] = ldg_keep_f4(gtab + split_gidx<K1, kSubM>(kA));
+        gB[kq] = ldg_keep_f4(gtab + split_gidx<K1, kSubM>((n - kA) & (n - 1)));
     }
     __syncwarp();
 #pragma unroll
@@ -483,7 +497,7 @@ __device__ __forceinline__ void split_sub256_pair(const Fft2Params &prm, const f
     if (special) {                                        // channel n/2 mirrors onto itself
         const cx<f2> zh = unpack_unit(mine[8]);
         cx<f2> rgA, rgB;
-        const cx<f2> gh = unpack_unit(__ldg(gtab + n / 2));
+        const cx<f2> gh = unpack_unit(__ldg(gtab + split_gidx<K1, kSubM>(n / 2)));
         rot_gain(8, gh, gh, rgA, rgB);
         split_epilogue<K1, F32OUT>(zh, zh, make_float2(1.0f, 0.0f), rgA, rgB, n / 2, n, stage, yout);
     }
@@ -598,6 +612,12 @@ struct SplitBigSmem {
     static constexpr size_t bytes = phase_off + sizeof(SplitPhaseBig);
 };
 
+// Output of the pair kernel: a transform ka holds the channels ka (mod 16), so a thread's int8 words are 64 bytes
+// apart and every 4-byte store is its own L2 sector; the eight CTAs of a spectrum run side by side and their words
+// meet in L2.  Collecting the words per eighth of the spectrum through a cluster's distributed shared memory
+// (st.shared::cluster into the owner CTA's staging buffer, one cluster barrier, then full-line stores) was built and
+// measured SLOWER (1.02 -> 1.70 ms for config 3: 4096 remote 4-byte stores per CTA at the ~20 B/clk of the SM-to-SM
+// network, plus the co-scheduling of 8-CTA clusters), so the direct stores stay.
 // grid (K1 / 2 pairs, spectra of the chunk, antennas); 2 * Plan::tpf threads
 template <class Plan, int K1, bool F32OUT>
 __global__ void __launch_bounds__(2 * Plan::tpf, 512 / (2 * Plan::tpf)) split_pair_kernel(const __grid_constant__ SplitParams sp)
@@ -646,14 +666,31 @@ __global__ void __launch_bounds__(2 * Plan::tpf, 512 / (2 * Plan::tpf)) split_pa
     const int k0 = ka + K1 * K;
     const float2 tpK = __ldg(prm.tpost + k0);
     const float4 *__restrict__ gtab = reinterpret_cast<const float4 *>(prm.rg2) + (int64_t)a * n;
-    uint32_t *rec = F32OUT ? nullptr : reinterpret_cast<uint32_t *>(prm.out + (((int64_t)a * prm.n_spectra + m) * n) * 4);
     float4 *yout = F32OUT ? reinterpret_cast<float4 *>(prm.out_f32 + (((int64_t)a * prm.n_spectra + m) * n) * 4) : nullptr;
+    uint32_t *rec = F32OUT ? nullptr : reinterpret_cast<uint32_t *>(prm.out + (((int64_t)a * prm.n_spectra + m) * n) * 4);
+    // post-twiddle, rotation x gain, quantisation and store of the pair (kA, kB)
+    auto finish = [&](cx<f2> zk, cx<f2> zm, float2 tp, cx<f2> rgA, cx<f2> rgB, int kA, int kB) {
+        const f2 sr = zk.re + zm.re, si = zk.im - zm.im;
+        const f2 dr = zk.re - zm.re, di = zk.im + zm.im;
+        const f2 fr = fnma_(di, tp.y, dr * tp.x);
+        const f2 fi = fma_(di, tp.x, dr * tp.y);
+        const cx<f2> xk = {sr - fr, si - fi};
+        const cx<f2> xm = {sr + fr, -(si + fi)};
+        const cx<f2> yA = cmul2(xk, rgA), yB = cmul2(xm, rgB);
+        if constexpr (F32OUT) {
+            yout[kA] = make_float4(yA.re.v.x, yA.im.v.x, yA.re.v.y, yA.im.v.y);
+            if (kB < n) yout[kB] = make_float4(yB.re.v.x, yB.im.v.x, yB.re.v.y, yB.im.v.y);
+        } else {
+            rec[kA] = quantize_unit(yA);
+            if (kB < n) rec[kB] = quantize_unit(yB);
+        }
+    };
     float4 gA[H], gB[H];
 #pragma unroll
     for (int kq = 0; kq < H; ++kq) {
         const int kA = k0 + K1 * Q * kq;
-        gA[kq] = ldg_keep_f4(gtab + kA);
-        gB[kq] = ldg_keep_f4(gtab + ((n - kA) & (n - 1)));
+        gA[kq] = ldg_keep_f4(gtab + split_gidx<K1, M>(kA));
+        gB[kq] = ldg_keep_f4(gtab + split_gidx<K1, M>((n - kA) & (n - 1)));
     }
     __syncthreads();                                           // upper halves are in the exchange buffers
     cx<f2> base = {f2(1.f, 1.f), f2(0.f, 0.f)};
@@ -685,14 +722,14 @@ __global__ void __launch_bounds__(2 * Plan::tpf, 512 / (2 * Plan::tpf)) split_pa
             const float cphi = w32_cos(kq * st), sphi = w32_sin(kq * st);
             tp = make_float2(fmaf(tpK.x, cphi, tpK.y * sphi), fmaf(-tpK.x, sphi, tpK.y * cphi));
         }
-        fft2_epilogue<F32OUT>(z[kq], zm, tp, rgA, rgB, kA, kB, n, rec, yout);
+        finish(z[kq], zm, tp, rgA, rgB, kA, kB);
     }
     if (special) {                                             // channel n/2 mirrors onto itself
         const cx<f2> zh = unpack_unit(mine[H]);
         cx<f2> rgA, rgB;
-        const cx<f2> gh = unpack_unit(__ldg(gtab + n / 2));
+        const cx<f2> gh = unpack_unit(__ldg(gtab + split_gidx<K1, M>(n / 2)));
         rot_gain(H, gh, gh, rgA, rgB);
-        fft2_epilogue<F32OUT>(zh, zh, make_float2(1.0f, 0.0f), rgA, rgB, n / 2, n, n, rec, yout);
+        finish(zh, zh, make_float2(1.0f, 0.0f), rgA, rgB, n / 2, n);
     }
 }
 

@@ -68,6 +68,7 @@ struct fengine {
     bool fft2p_attr[2] = {};
     int opt_split = -1;             // option "split" (fe_split.cuh): -1 = where it wins (n >= 16384), 0 = never, 1 = wherever it exists
     float2 *d_sp_tw1 = nullptr, *d_sp_tw256 = nullptr;   // its twiddle tables
+    float4 *d_rg2s = nullptr;                            // d_rg2 in split order (fe_split.cuh: split_gidx)
     float2 *d_sp_ptw1 = nullptr, *d_sp_ptw2 = nullptr;   // n >= 16384: pass twiddles of the n/16-point plan of the pair kernel
     bool split_attr[3] = {};        // shared-memory attribute set (producer, consumer int8, consumer f32)
     int ring_rows = 32;             // option "ring_rows" (D: rows per track, a power of two >= 16)
@@ -557,6 +558,7 @@ int refresh_tables(fengine *fe)
         dim3 grid((unsigned)((fe->n + 255) / 256), (unsigned)fe->A);
         build_rg2_table<<<grid, 256>>>(fe->d_rg2, fe->d_gains, fe->d_coarse, fe->d_fine_d, fe->d_fine_phi, fe->n, fe->A, mode);
         fe->rg2_mode = mode;
+        if (fe->d_rg2s) permute_rg2_split<<<grid, 256>>>(fe->d_rg2s, fe->d_rg2, fe->n, 16, fe->A);
     }
     FE_CUDA(fe, cudaGetLastError());
     FE_CUDA(fe, cudaDeviceSynchronize());
@@ -758,6 +760,7 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
             SplitParams sp{};
             sp.fir = fp2;
             sp.fft = xp2;
+            sp.fft.rg2 = fe->d_rg2s;
             sp.fir.rows_per_tile = split_rows_for(fe, m1 - m0);
             sp.tw1 = fe->d_sp_tw1;
             sp.tw256 = fe->d_sp_tw256;
@@ -871,6 +874,7 @@ try {
             bool okm = cudaMalloc(&fe->d_sp_tw1, sizeof(float2) * (size_t)K1 * M) == cudaSuccess &&
                        cudaMalloc(&fe->d_sp_tw256, sizeof(float2) * 256) == cudaSuccess;
             if (okm && !fe->d_rg2) okm = cudaMalloc(&fe->d_rg2, sizeof(float4) * (size_t)fe->A * fe->n) == cudaSuccess;
+            if (okm) okm = cudaMalloc(&fe->d_rg2s, sizeof(float4) * (size_t)fe->A * fe->n) == cudaSuccess;
             if (okm) {
                 build_scalar_twiddles<<<(K1 * M + 255) / 256, 256>>>(fe->d_sp_tw1, K1, M, fe->n);
                 build_scalar_twiddles<<<1, 256>>>(fe->d_sp_tw256, 16, 16, 256);
@@ -927,6 +931,7 @@ void fengine_destroy(fengine_t *fe)
     cudaFree(fe->d_rg2);
     cudaFree(fe->d_sp_tw1);
     cudaFree(fe->d_sp_tw256);
+    cudaFree(fe->d_rg2s);
     cudaFree(fe->d_sp_ptw1);
     cudaFree(fe->d_sp_ptw2);
     cudaFree(fe->d_scratch);
