@@ -225,8 +225,8 @@ int fengine_debug_pipe_stats(fengine_t *fe, uint64_t *out, int64_t max_words);
 enum {
     FENGINE_PATH_GENERIC = 0,                 /* one thread per output (any shape; slow, for tests) */
     FENGINE_PATH_ONE_POL = 1,                 /* fe_fir.cuh + fe_fft.cuh */
-    FENGINE_PATH_POL_PACKED = 2,              /* fe_fir2.cuh / fe_fir2b.cuh / fe_fir3.cuh + fe_fft2.cuh */
-    FENGINE_PATH_PACKED_FIR_ONE_POL_FFT = 3,  /* fe_fir2b.cuh / fe_fir3.cuh + fe_fft.cuh (n >= 16384: 32 taps, other sample widths) */
+    FENGINE_PATH_POL_PACKED = 2,              /* fe_fir2.cuh / fe_fir3.cuh + fe_fft2.cuh */
+    FENGINE_PATH_PACKED_FIR_ONE_POL_FFT = 3,  /* fe_fir2.cuh / fe_fir3.cuh + fe_fft.cuh (n >= 16384: 32 taps, other sample widths) */
     FENGINE_PATH_FUSED = 4,                   /* fe_pipe.cuh */
     FENGINE_PATH_SPLIT = 5                    /* fe_split.cuh */
 };

@@ -16,6 +16,8 @@
 #pragma once
 #include <cuda_fp16.h>
 
+#include <type_traits>
+
 #include "fe_common.cuh"
 #include "fe_fir.cuh"
 
@@ -37,8 +39,22 @@ struct Fir2Params {
 
 constexpr int kFir2Threads = 128;
 constexpr int kFir2Warps = kFir2Threads / 32;
-constexpr int kFir2SegBytes = 80;                                   // per warp per row per pol: 16 groups x 5 bytes
-constexpr int kFir2SlotBytes = 2 * kFir2SegBytes;                   // both pols
+
+// BITS = sample width of the packed input (10 in the paper's deployment; 4 / 8 / 12 / 16 are its
+// bit-depth sweep): same big-endian bit stream, sample u in bits [BITS u, BITS u + BITS).  A warp's
+// row segment (64 samples per pol) is 8 BITS bytes, a thread's two samples are 2 BITS bits at bit 2 BITS lane.  The
+// geometry of the packed row is the only thing the width changes; arithmetic, partial sums, rotation and the scratch
+// layouts are one piece of code (fir2_run).
+template <int BITS> struct Fir2Geom {
+    static constexpr int seg = 8 * BITS;                              // bytes per warp, row and pol
+    static constexpr int slot = 2 * seg;                              // both pols
+    static constexpr int cpp = BITS / 2;                              // 16-byte chunks per pol segment
+    static constexpr int batch_chunks = 4 * 2 * cpp;                  // kFirBatch rows x 2 pols
+    static_assert(BITS == 4 || BITS == 8 || BITS == 10 || BITS == 12 || BITS == 16, "sample width");
+    static_assert(batch_chunks <= 64, "at most two chunks per lane and batch");
+};
+constexpr int kFir2SegBytes = Fir2Geom<10>::seg;                    // 80: 16 groups x 5 bytes
+constexpr int kFir2SlotBytes = Fir2Geom<10>::slot;
 
 // Where the finished rows of a run go.  A sink sees, for every step s = 0, 1, .. of the run, one call of
 // store(cur) (the 16-byte unit of this thread's point for the run-relative row sp = s - T + lag, which the sink
@@ -82,13 +98,37 @@ struct Fir2ScratchSinkH16 {
     }
 };
 
+// Scratch in the layout of the one-pol FFT (fe_fft.cuh: a row of N floats per (antenna, spectrum, pol), every four
+// columns stored as (g0, g2, g1, g3)): point i = 2 q + e holds the columns 4 q + 2 e (Re z, stored at 4 q + e) and
+// 4 q + 2 e + 1 (Im z, stored at 4 q + 2 + e); gp points at the pol-0 row, pol 1 is the next row.  Used where the
+// pol-packed FFT has no plan (n >= 16384) so that the sweeps of PAPER.md:245 and :273-279 still run a tiled FIR.
+struct Fir2OnePolSink {
+    float *gp;
+    size_t g_stride;
+    int N;
+    int sp, n_out;
+    __device__ __forceinline__ void begin_run(int lag, int T, int n_out_) { gp += ((int64_t)lag - T) * (int64_t)g_stride; sp = lag - T; n_out = n_out_; }
+    __device__ __forceinline__ void before_steps(int) {}
+    __device__ __forceinline__ void after_steps(int) {}
+    __device__ __forceinline__ void end_run() {}
+    __device__ __forceinline__ void store(float4 cur)
+    {
+        asm volatile("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %6, %7;\n\t@p st.global.f32 [%0], %2;\n\t@p st.global.f32 [%0+8], %4;\n\t"
+                     "@p st.global.f32 [%1], %3;\n\t@p st.global.f32 [%1+8], %5;\n\t}"
+                     ::"l"(gp), "l"(gp + N), "f"(cur.x), "f"(cur.y), "f"(cur.z), "f"(cur.w), "r"((unsigned)sp), "r"((unsigned)n_out) : "memory");
+        gp += g_stride;
+        ++sp;
+    }
+};
+
 // Ring step q holds input row R0 + q of both pols, R0 = m0 - cq - 1; see fir_run in fe_fir.cuh for the
 // partial-sum bookkeeping, which is identical.
 // NC: the row width N when the caller knows it at compile time (row strides become immediates), else 0.
-template <int T, bool MIXED, class Sink, int NC = 0>
+template <int T, bool MIXED, class Sink, int NC = 0, int BITS = 10>
 __device__ __forceinline__ void fir2_run(const Fir2Params &prm, const uint8_t *wsrc, uint32_t ring_s, int64_t c,
                                          int64_t m0, int n_out, int i_pt, Sink &sink)
 {
+    using G = Fir2Geom<BITS>;
     constexpr int U = kFirUnroll;
     static_assert(U % T == 0 && U % kFirDepth == 0, "unroll must cover whole tap and ring periods");
     const int N = NC ? NC : 1 << prm.lgN;
@@ -115,23 +155,24 @@ __device__ __forceinline__ void fir2_run(const Fir2Params &prm, const uint8_t *w
     }
     const int lag0 = lagc[0] ? 1 : 0;
     const int64_t R0 = m0 - cq - 1;
-    const int row_bytes = N / 4 * 5;
+    const int row_bytes = N / 8 * BITS;
 
-    // this thread's bytes in a slot: group gi = lane/2 of the warp's 16 groups, point e = lane&1 of the
-    // group: bytes [5 gi + e, 5 gi + e + 4) hold its two samples (bits 39..20 for e = 0, 19..0 for e = 1)
-    const int e = lane & 1;
-    const uint32_t boff = (uint32_t)(5 * (lane >> 1) + e);
+    // this thread's bits in a slot: 2 BITS bits at bit 2 BITS lane of the warp's segment; b0..b3 = the four bytes
+    // that start at byte boff, after sha leading bits (sha + 2 BITS <= 32 for every supported width)
+    const uint32_t bit0 = 2u * BITS * (uint32_t)lane;
+    const uint32_t boff = bit0 >> 3;
     const uint32_t sh = boff & 3;
     const uint32_t sel = (sh + 3) | ((sh + 2) << 4) | ((sh + 1) << 8) | (sh << 12);
     const uint32_t rd_addr = ring_s + (boff >> 2) * 4u;          // W0 of pol 0 in slot 0
-    const uint32_t sha = e ? 12u : 0u;                           // left shift that brings sample a to bits 31..22
+    const uint32_t sha = bit0 & 7u;                              // left shift that brings sample a to the top bits
 
-    // Batch copy: 4 rows x 2 pols x 5 chunks of 16 bytes = 40 chunks; lane l moves chunk l, lanes 0..7 also 32+l.
-    const int rowA = lane / 10, remA = lane - rowA * 10, polA = remA / 5, colA = remA - polA * 5;
-    const bool hasB = lane < 8;
-    const int rowB = 3, remB = hasB ? 2 + lane : 0, polB = remB / 5, colB = remB - polB * 5;
-    const uint32_t dstA = ring_s + (uint32_t)(rowA * kFir2SlotBytes + polA * kFir2SegBytes + colA * 16);
-    const uint32_t dstB = ring_s + (uint32_t)(rowB * kFir2SlotBytes + polB * kFir2SegBytes + colB * 16);
+    // Batch copy: 4 rows x 2 pols x cpp chunks of 16 bytes; lane l moves chunk l and, where it exists, chunk 32 + l.
+    const int idxA = lane, idxB = 32 + lane;
+    const bool hasA = idxA < G::batch_chunks, hasB = idxB < G::batch_chunks;
+    const int rowA = hasA ? idxA / (2 * G::cpp) : 0, remA = hasA ? idxA % (2 * G::cpp) : 0, polA = remA / G::cpp, colA = remA % G::cpp;
+    const int rowB = hasB ? idxB / (2 * G::cpp) : 0, remB = hasB ? idxB % (2 * G::cpp) : 0, polB = remB / G::cpp, colB = remB % G::cpp;
+    const uint32_t dstA = ring_s + (uint32_t)(rowA * G::slot + polA * G::seg + colA * 16);
+    const uint32_t dstB = ring_s + (uint32_t)(rowB * G::slot + polB * G::seg + colB * 16);
     const uint8_t *srcA = wsrc + polA * prm.stream_bytes + (R0 + rowA) * (int64_t)row_bytes + colA * 16;
     const uint8_t *srcB = wsrc + polB * prm.stream_bytes + (R0 + rowB) * (int64_t)row_bytes + colB * 16;
     const int64_t batch_bytes = (int64_t)kFirBatch * row_bytes;
@@ -144,8 +185,8 @@ __device__ __forceinline__ void fir2_run(const Fir2Params &prm, const uint8_t *w
     auto issue_batch = [&](int slot0) {
         const uint32_t okA = (uint32_t)tA < span ? 1u : 0u;
         const uint32_t okB = (uint32_t)tB < span ? 1u : 0u;
-        ring_fill(dstA + slot0 * kFir2SlotBytes, srcA, okA, okA ^ 1u);
-        ring_fill(dstB + slot0 * kFir2SlotBytes, srcB, hasB ? okB : 0u, hasB ? (okB ^ 1u) : 0u);
+        ring_fill(dstA + slot0 * G::slot, srcA, hasA ? okA : 0u, hasA ? (okA ^ 1u) : 0u);
+        ring_fill(dstB + slot0 * G::slot, srcB, hasB ? okB : 0u, hasB ? (okB ^ 1u) : 0u);
         asm volatile("cp.async.commit_group;" ::: "memory");
         srcA += batch_bytes;
         srcB += batch_bytes;
@@ -168,11 +209,11 @@ __device__ __forceinline__ void fir2_run(const Fir2Params &prm, const uint8_t *w
     // ii + 1 are read from the ring while the FMAs of step ii issue, and the scratch store is a predicated
     // instruction, so the unpack chain (LDS -> PRMT -> SHF -> I2FP) of the next step hides behind 32 FFMA2s.
     auto load_raw = [&](int slot, uint32_t (&raw)[4]) {
-        const uint32_t ad = rd_addr + slot * kFir2SlotBytes;
+        const uint32_t ad = rd_addr + slot * G::slot;
         asm volatile("ld.shared.u32 %0, [%1];" : "=r"(raw[0]) : "r"(ad) : "memory");
         asm volatile("ld.shared.u32 %0, [%1+4];" : "=r"(raw[1]) : "r"(ad) : "memory");
-        asm volatile("ld.shared.u32 %0, [%1+80];" : "=r"(raw[2]) : "r"(ad) : "memory");
-        asm volatile("ld.shared.u32 %0, [%1+84];" : "=r"(raw[3]) : "r"(ad) : "memory");
+        asm volatile("ld.shared.u32 %0, [%1+%2];" : "=r"(raw[2]) : "r"(ad), "n"(G::seg) : "memory");
+        asm volatile("ld.shared.u32 %0, [%1+%2];" : "=r"(raw[3]) : "r"(ad), "n"(G::seg + 4) : "memory");
     };
     uint32_t nxt[4];
     cp_async_wait<kFirRingBatches - 2>();
@@ -194,10 +235,10 @@ __device__ __forceinline__ void fir2_run(const Fir2Params &prm, const uint8_t *w
                 issue_batch((((ii + 1) / kFirBatch + kFirRingBatches - 1) % kFirRingBatches) * kFirBatch);
             }
             load_raw((ii + 1) % kFirDepth, nxt);
-            const uint32_t be0 = __byte_perm(P0a, P0b, sel) << sha;     // sample a in bits 31..22, b in 21..12
+            const uint32_t be0 = __byte_perm(P0a, P0b, sel) << sha;     // sample a in the top BITS bits, b below it
             const uint32_t be1 = __byte_perm(P1a, P1b, sel) << sha;
-            const f2 s0((float)((int32_t)be0 >> 22), (float)((int32_t)be1 >> 22));                  // column v0, (p0, p1)
-            const f2 s1((float)((int32_t)(be0 << 10) >> 22), (float)((int32_t)(be1 << 10) >> 22));  // column v0 + 1
+            const f2 s0((float)((int32_t)be0 >> (32 - BITS)), (float)((int32_t)be1 >> (32 - BITS)));                    // column v0, (p0, p1)
+            const f2 s1((float)((int32_t)(be0 << BITS) >> (32 - BITS)), (float)((int32_t)(be1 << BITS) >> (32 - BITS)));  // column v0 + 1
             // one column at a time: consecutive FFMA2s then share the sample operand, which ptxas keeps in the
             // operand-reuse cache (a FFMA2 with three fresh register operands issues at ~77 % of the packed rate,
             // measured; with the sample reused it issues at ~96 %)
@@ -225,11 +266,15 @@ __device__ __forceinline__ void fir2_run(const Fir2Params &prm, const uint8_t *w
     sink.end_run();
 }
 
-template <int T, bool H16 = false>
+// OUT: where the finished rows go
+enum { kFir2OutPacked = 0, kFir2OutPackedH16 = 1, kFir2OutOnePol = 2 };
+
+template <int T, int OUT = kFir2OutPacked, int BITS = 10>
 __global__ void __launch_bounds__(kFir2Threads, 4) fir2_kernel(const Fir2Params prm)
 {
+    using G = Fir2Geom<BITS>;
     // +16: the second word of the last lane's pol-1 group may lie just past the last slot (never selected)
-    __shared__ __align__(16) unsigned char ring_all[kFir2Warps * kFirDepth * kFir2SlotBytes + 16];
+    __shared__ __align__(16) unsigned char ring_all[kFir2Warps * kFirDepth * G::slot + 16];
     const int N = 1 << prm.lgN;
     const int a = blockIdx.z;
     const int warp = threadIdx.x >> 5;
@@ -237,9 +282,9 @@ __global__ void __launch_bounds__(kFir2Threads, 4) fir2_kernel(const Fir2Params 
     int64_t m = prm.m_begin + (int64_t)blockIdx.y * prm.rows_per_tile;
     const int64_t m_stop = min(m + (int64_t)prm.rows_per_tile, prm.m_end);
     const uint8_t *sbase = prm.in + (int64_t)a * 2 * prm.stream_bytes;
-    const uint8_t *wsrc = sbase + (int64_t)(blockIdx.x * kFir2Warps + warp) * kFir2SegBytes;
+    const uint8_t *wsrc = sbase + (int64_t)(blockIdx.x * kFir2Warps + warp) * G::seg;
     const int32_t *ctab = prm.coarse + (int64_t)a * 2 * prm.n_coarse;
-    const uint32_t ring_s = (uint32_t)__cvta_generic_to_shared(ring_all + warp * kFirDepth * kFir2SlotBytes);
+    const uint32_t ring_s = (uint32_t)__cvta_generic_to_shared(ring_all + warp * kFirDepth * G::slot);
 
     while (m < m_stop) {
         const int32_t c = ctab[prm.n_coarse == 1 ? 0 : m];
@@ -250,22 +295,24 @@ __global__ void __launch_bounds__(kFir2Threads, 4) fir2_kernel(const Fir2Params 
         }
         const int cr = (int)((int64_t)c & (int64_t)(N - 1));
         const bool mixed = (2 * i_pt + cr < N) && (2 * i_pt + 1 + cr >= N);
-        if constexpr (H16) {
-            float *grow0 = prm.g + ((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * (int64_t)N;
-            Fir2ScratchSinkH16 sink{grow0 + 2 * i_pt, (size_t)N, 0, 0};
+        const int n_run = (int)(run_end - m);
+        const int64_t row = (int64_t)a * prm.chunk_cap + (m - prm.m_begin);
+        auto run = [&](auto &sink) {
             if (__any_sync(0xffffffffu, mixed))
-                fir2_run<T, true>(prm, wsrc, ring_s, (int64_t)c, m, (int)(run_end - m), i_pt, sink);
+                fir2_run<T, true, std::remove_reference_t<decltype(sink)>, 0, BITS>(prm, wsrc, ring_s, (int64_t)c, m, n_run, i_pt, sink);
             else
-                fir2_run<T, false>(prm, wsrc, ring_s, (int64_t)c, m, (int)(run_end - m), i_pt, sink);
-            m = run_end;
-            continue;
+                fir2_run<T, false, std::remove_reference_t<decltype(sink)>, 0, BITS>(prm, wsrc, ring_s, (int64_t)c, m, n_run, i_pt, sink);
+        };
+        if constexpr (OUT == kFir2OutPackedH16) {               // 8-byte units: a row is N floats wide
+            Fir2ScratchSinkH16 sink{prm.g + row * (int64_t)N + 2 * i_pt, (size_t)N, 0, 0};
+            run(sink);
+        } else if constexpr (OUT == kFir2OutOnePol) {           // rows (antenna, spectrum, pol) of N floats
+            Fir2OnePolSink sink{prm.g + row * (int64_t)N * 2 + 4 * (i_pt >> 1) + (i_pt & 1), (size_t)N * 2, N, 0, 0};
+            run(sink);
+        } else {
+            Fir2ScratchSink sink{prm.g + row * (int64_t)N * 2 + 4 * i_pt, (size_t)N * 2, 0, 0};
+            run(sink);
         }
-        float *grow0 = prm.g + ((int64_t)a * prm.chunk_cap + (m - prm.m_begin)) * (int64_t)N * 2;
-        Fir2ScratchSink sink{grow0 + 4 * i_pt, (size_t)N * 2, 0, 0};
-        if (__any_sync(0xffffffffu, mixed))
-            fir2_run<T, true>(prm, wsrc, ring_s, (int64_t)c, m, (int)(run_end - m), i_pt, sink);
-        else
-            fir2_run<T, false>(prm, wsrc, ring_s, (int64_t)c, m, (int)(run_end - m), i_pt, sink);
         m = run_end;
     }
 }

@@ -21,7 +21,6 @@
 #include "fe_fft2.cuh"
 #include "fe_fir.cuh"
 #include "fe_fir2.cuh"
-#include "fe_fir2b.cuh"
 #include "fe_fir3.cuh"
 #include "fe_generic.cuh"
 #include "fe_pipe.cuh"
@@ -231,7 +230,7 @@ int launch_fft2_n(fengine *fe, const Fft2Params &prm, int64_t chunk_len, cudaStr
 }
 
 // Shapes the pol-packed FFT does not cover (n >= 16384) but a pol-packed FIR does: 32 taps (fe_fir3.cuh) and sample
-// widths other than 10 bits with 16 taps (fe_fir2b.cuh) write the scratch in the one-pol FFT's layout, so the tap and
+// widths other than 10 bits with 16 taps (fe_fir2.cuh with another sample width) write the scratch in the one-pol FFT's layout, so the tap and
 // bit-depth sweeps of the paper (both at 32768 channels) run tiled kernels end to end.
 bool use_packed_fir_onepol_fft(const fengine *fe)
 {
@@ -380,19 +379,19 @@ int launch_fir2(fengine *fe, const Fir2Params &prm, int64_t chunk_len, cudaStrea
     if (fe->bits != 10) {                                   // bit-depth sweep: 16 taps only
         if (onepol) {
             switch (fe->bits) {
-            case 4: fir2b_kernel<16, 4, true><<<grid, kFir2Threads, 0, stream>>>(prm); break;
-            case 8: fir2b_kernel<16, 8, true><<<grid, kFir2Threads, 0, stream>>>(prm); break;
-            case 12: fir2b_kernel<16, 12, true><<<grid, kFir2Threads, 0, stream>>>(prm); break;
-            case 16: fir2b_kernel<16, 16, true><<<grid, kFir2Threads, 0, stream>>>(prm); break;
+            case 4: fir2_kernel<16, kFir2OutOnePol, 4><<<grid, kFir2Threads, 0, stream>>>(prm); break;
+            case 8: fir2_kernel<16, kFir2OutOnePol, 8><<<grid, kFir2Threads, 0, stream>>>(prm); break;
+            case 12: fir2_kernel<16, kFir2OutOnePol, 12><<<grid, kFir2Threads, 0, stream>>>(prm); break;
+            case 16: fir2_kernel<16, kFir2OutOnePol, 16><<<grid, kFir2Threads, 0, stream>>>(prm); break;
             default: return fail(fe, FENGINE_ERR_INVALID_ARG, "no tiled FIR for %d-bit samples", fe->bits);
             }
             return FENGINE_OK;
         }
         switch (fe->bits) {
-        case 4: fir2b_kernel<16, 4><<<grid, kFir2Threads, 0, stream>>>(prm); break;
-        case 8: fir2b_kernel<16, 8><<<grid, kFir2Threads, 0, stream>>>(prm); break;
-        case 12: fir2b_kernel<16, 12><<<grid, kFir2Threads, 0, stream>>>(prm); break;
-        case 16: fir2b_kernel<16, 16><<<grid, kFir2Threads, 0, stream>>>(prm); break;
+        case 4: fir2_kernel<16, kFir2OutPacked, 4><<<grid, kFir2Threads, 0, stream>>>(prm); break;
+        case 8: fir2_kernel<16, kFir2OutPacked, 8><<<grid, kFir2Threads, 0, stream>>>(prm); break;
+        case 12: fir2_kernel<16, kFir2OutPacked, 12><<<grid, kFir2Threads, 0, stream>>>(prm); break;
+        case 16: fir2_kernel<16, kFir2OutPacked, 16><<<grid, kFir2Threads, 0, stream>>>(prm); break;
         default: return fail(fe, FENGINE_ERR_INVALID_ARG, "no tiled FIR for %d-bit samples", fe->bits);
         }
         return FENGINE_OK;
@@ -404,7 +403,7 @@ int launch_fir2(fengine *fe, const Fir2Params &prm, int64_t chunk_len, cudaStrea
     case 8: fir2_kernel<8><<<grid, kFir2Threads, 0, stream>>>(prm); break;
     case 16:
         if (fe->scratch_h16)
-            fir2_kernel<16, true><<<grid, kFir2Threads, 0, stream>>>(prm);
+            fir2_kernel<16, kFir2OutPackedH16><<<grid, kFir2Threads, 0, stream>>>(prm);
         else if (fe->l2_persist)
             FE_CUDA(fe, launch_win(fir2_kernel<16>, grid, dim3(kFir2Threads), 0, stream, &fe->l2_win, prm));
         else

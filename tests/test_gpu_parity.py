@@ -339,7 +339,7 @@ def test_streaming_pushes_equal_one_batch(torch, fb, n, T, A, crange, pushes, eq
 ])
 def test_tap_and_bit_depth_sweeps_run_tiled_kernels_at_large_n(torch, fb, n, T, bits, S, A):
     """SURVEY.md 8(f2) at the survey's size: 32 taps and 4 / 8 / 12 / 16-bit samples at n >= 16384 run a pol-packed FIR
-    (fe_fir3.cuh / fe_fir2b.cuh) that writes the one-pol FFT's scratch layout, not the one-thread-per-output kernels."""
+    (fe_fir3.cuh / fe_fir2.cuh) that writes the one-pol FFT's scratch layout, not the one-thread-per-output kernels."""
     sigma = {4: 2.0, 8: 30.0, 10: 32.0, 12: 400.0, 16: 6000.0}[bits]
     w = si.custom_workload(A=A, n=n, T=T, S=S, P=2, seed=71, coarse_range=(-3 * n, 5 * n), bits=bits, sigma=sigma)
     w.coarse[:, 1] = w.coarse[:, 0]
