@@ -670,6 +670,44 @@ def test_rank_local_engines_reproduce_the_full_engine(torch, fb):
     np.testing.assert_array_equal(np.concatenate(parts, axis=0), full)
 
 
+def _random_case(seed):
+    rng = np.random.default_rng(1000 + seed)
+    n = int(rng.choice([1024, 2048, 4096, 8192, 16384, 32768]))
+    T = int(rng.choice([2, 4, 8, 16, 32] if n <= 8192 else [2, 4, 8, 16]))
+    A = int(rng.integers(1, 4))
+    S = int(rng.integers(1, 70 if n <= 8192 else 30))
+    per_spectrum = bool(rng.integers(2))
+    equal_pols = bool(rng.integers(4))                      # three in four: the pol-packed / split kernels
+    opts = {}
+    if rng.integers(2):
+        opts["chunk_spectra"] = int(rng.integers(1, S + 1))
+    if rng.integers(2):
+        opts["fir_rows"] = int(rng.integers(1, 80))
+    if T != 32:
+        pick = int(rng.integers(4))
+        if pick == 1:
+            opts["split"] = int(rng.integers(0, 2))
+        elif pick == 2 and n <= 4096:
+            opts["fft_persistent"] = 1
+        elif pick == 3 and n <= 8192:
+            opts["fused"] = 1
+    return n, T, A, S, per_spectrum, equal_pols, opts
+
+
+@pytest.mark.parametrize("seed", range(24))
+def test_random_shapes_and_options(torch, fb, seed):
+    """Seeded random shapes, delay modes and path options against the oracle: every path must agree, whatever ran."""
+    n, T, A, S, per_spectrum, equal_pols, opts = _random_case(seed)
+    w = si.custom_workload(A=A, n=n, T=T, S=S, P=2, seed=200 + seed, per_spectrum=per_spectrum, coarse_range=(-2 * n, 4 * n))
+    if equal_pols:
+        w.coarse[:, 1] = w.coarse[:, 0]
+    fe = make_engine(fb, w, **opts)
+    got = gpu_run(torch, fe, w)
+    check_parity(got, oracle_run(w), f"seed {seed}: n={n} T={T} A={A} S={S} per_spectrum={per_spectrum} equal={equal_pols} {opts} path={fe.path()}")
+    again = gpu_run(torch, fe, w, want=("int8",))["out"]      # and a second call on the same handle is identical
+    np.testing.assert_array_equal(again, got["out"])
+
+
 def test_setters_take_effect_between_calls(torch, fb):
     w = si.make_workload(1, n_spectra=10)
     fe = make_engine(fb, w)
