@@ -157,6 +157,39 @@ static __global__ void heaps_transpose_kernel(const Word *__restrict__ rec, Word
 }
 
 
+// The same transposition for 4-byte words (two pols) and n a multiple of 64: 64 x 64-word tiles, 256 threads, every
+// global access 16 bytes wide (four channels on the way in, four spectra on the way out), 256 contiguous bytes per
+// 16 lanes on both sides; the tile rows are 65 words apart so that neither phase has a bank conflict.
+static __global__ void __launch_bounds__(256) heaps_transpose64_kernel(const uint32_t *__restrict__ rec, uint32_t *__restrict__ heaps,
+                                                                      int64_t S, int n)
+{
+    __shared__ uint32_t tile[64][65];
+    const int64_t n_heaps = (S + 255) / 256;
+    const int a = blockIdx.z / (int)n_heaps, h = blockIdx.z - a * (int)n_heaps;
+    const int k0 = blockIdx.x * 64, s0 = blockIdx.y * 64;             // channel / in-heap spectrum of the tile
+    const uint32_t *src = rec + ((int64_t)a * S + (int64_t)h * 256) * n;
+    uint32_t *dst = heaps + ((int64_t)a * n_heaps + h) * (int64_t)n * 256;
+    const int q = threadIdx.x & 15, r = threadIdx.x >> 4;
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+        const int j = r + 16 * p;                                     // spectrum of the tile
+        const int64_t m = (int64_t)h * 256 + s0 + j;
+        uint4 v = make_uint4(0u, 0u, 0u, 0u);
+        if (m < S) v = *reinterpret_cast<const uint4 *>(src + (int64_t)(s0 + j) * n + k0 + 4 * q);
+        tile[j][4 * q] = v.x;
+        tile[j][4 * q + 1] = v.y;
+        tile[j][4 * q + 2] = v.z;
+        tile[j][4 * q + 3] = v.w;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+        const int c = r + 16 * p;                                     // channel of the tile
+        const uint4 v = make_uint4(tile[4 * q][c], tile[4 * q + 1][c], tile[4 * q + 2][c], tile[4 * q + 3][c]);
+        stg_stream_u4(reinterpret_cast<uint4 *>(dst + (int64_t)(k0 + c) * 256 + s0 + 4 * q), v);
+    }
+}
+
 // Measurement hook (fengine_debug_fp32_rate): the FIR's instruction form, one sample pair against 16 scalar weights
 // into 16 accumulator pairs (FFMA2, the sample operand reused), in a loop that does nothing else.  What it sustains is
 // the denominator of the "alu" roofline of bench.py; the path's butterflies (FADD2 / FMUL2)

@@ -1105,7 +1105,10 @@ try {
     if (rc) return rc;
     const int64_t n_heaps = (n_spectra + 255) / 256;
     dim3 grid((unsigned)(fe->n / 32), 8, (unsigned)(fe->A * n_heaps)), block(32, 8);
-    if (fe->P == 2)
+    if (fe->P == 2 && fe->n % 64 == 0)
+        heaps_transpose64_kernel<<<dim3((unsigned)(fe->n / 64), 4, (unsigned)(fe->A * n_heaps)), 256, 0, s>>>(
+            reinterpret_cast<const uint32_t *>(fe->d_rec), static_cast<uint32_t *>(heaps_out), n_spectra, fe->n);
+    else if (fe->P == 2)
         heaps_transpose_kernel<uint32_t><<<grid, block, 0, s>>>(reinterpret_cast<const uint32_t *>(fe->d_rec),
                                                                 static_cast<uint32_t *>(heaps_out), n_spectra, fe->n);
     else
