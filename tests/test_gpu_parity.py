@@ -708,6 +708,36 @@ def test_random_shapes_and_options(torch, fb, seed):
     np.testing.assert_array_equal(again, got["out"])
 
 
+@pytest.mark.parametrize("cfg,opts", [(2, {}), (2, {"split": 1}), (1, {})])
+def test_reserve_makes_process_allocation_free_and_capturable(torch, fb, cfg, opts):
+    """fengine_reserve ("the library never allocates in this call"): after it a larger call is refused
+    with FENGINE_ERR_STATE instead of allocating, and a call can be captured into a CUDA graph and replayed."""
+    w = si.make_workload(cfg, n_spectra=40, n_antennas=1)
+    fe = make_engine(fb, w, **opts)
+    fe.reserve(w.S)
+    d_in = torch.from_numpy(w.packed.reshape(-1)).cuda()
+    d_out = torch.zeros(fe.output_shape(w.S), dtype=torch.int8, device="cuda")
+    fe.process(d_in, d_out, w.S)                                  # first call: kernel attributes are set here
+    torch.cuda.synchronize()
+    ref = oracle_run(w)
+    check_parity({"out": d_out.cpu().numpy()}, ref, "reserved")
+    big_in = torch.zeros(fe.input_bytes(2 * w.S), dtype=torch.uint8, device="cuda")
+    big_out = torch.zeros(fe.output_shape(2 * w.S), dtype=torch.int8, device="cuda")
+    with pytest.raises(fb.FEngineError) as e:
+        fe.process(big_in, big_out, 2 * w.S)
+    assert e.value.code == 4
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(g, stream=side):
+            fe.process(d_in, d_out, w.S, stream=side.cuda_stream)
+    d_out.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    check_parity({"out": d_out.cpu().numpy()}, ref, "graph replay")
+
+
 def test_setters_take_effect_between_calls(torch, fb):
     w = si.make_workload(1, n_spectra=10)
     fe = make_engine(fb, w)
