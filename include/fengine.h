@@ -187,9 +187,10 @@ int fengine_debug_fir(fengine_t *fe, const void *in, float *g_out, int64_t n_spe
  * antenna in packed FP32 lanes; they are used when n_pols = 2, n <= 8192 and the two pols of every antenna have
  * equal coarse delays), "fused" (0/1, default 0: run the pol-packed path as ONE persistent, warp-specialised kernel
  * whose FIR -> FFT transposition goes through an L2-resident ring of rows instead of a full-size HBM scratch,
- * fe_pipe.cuh; T = 2, 4, 8, 16; knobs "ring_rows", "fir_warps", "tracks", "segments", "pipe_ctas"), "split" (0/1,
- * default 0, n = 4096: the first radix-16 stage of the transform runs in the FIR kernel and the rest as independent
- * 256-point transforms per warp, fe_split.cuh, the arrangement PAPER.md:403-409 proposes), "fft_persistent" (0/1, default 0: the
+ * fe_pipe.cuh; T = 2, 4, 8, 16; knobs "ring_rows", "fir_warps", "tracks", "segments", "pipe_ctas"), "split" (-1 / 0 / 1,
+ * n = 4096, 16384, 32768, equal coarse delays in both pols: the first radix-16 stage of the transform runs in the FIR
+ * kernel and the rest as independent n/16-point transforms, fe_split.cuh, the arrangement PAPER.md:403-409 proposes;
+ * -1 (default) = where it measures faster, i.e. n >= 16384, 0 = never, 1 = wherever it exists), "fft_persistent" (0/1, default 0: the
  * pol-packed FFT as one persistent CTA per SM whose rows arrive by bulk copy into the exchange buffer, n <= 4096),
  * "scratch_fp16" (0/1, default 0; T = 16, n = 1024 or 4096, pol-packed path: the FIR output / FFT input is stored in
  * FP16 with FP32 arithmetic on both sides, the variant PAPER.md:407 proposes; NOT within the 1e-4 parity bar, it is

@@ -1,24 +1,25 @@
 // fe_split.cuh -- the pol-packed path split the way the paper's conclusion proposes ("step 2 of the
-// six-step FFT merged into the PFB FIR kernel"): the n-point complex transform of a spectrum is n = K1 * 256,
+// six-step FFT merged into the PFB FIR kernel"): the n-point complex transform of a spectrum is n = 16 M,
 //
-//   stage 1 (producer, with the FIR)   y[ka][i'] = W_n^{i' ka} * sum_{q < K1} z[i' + 256 q] W_K1^{q ka}       (ka < K1, i' < 256)
-//   stage 2 (consumer)                 Z[ka + K1 k'] = sum_{i' < 256} y[ka][i'] W_256^{i' k'}                 (k' < 256)
+//   stage 1 (producer, with the FIR)   y[ka][i'] = W_n^{i' ka} * sum_{q < 16} z[i' + M q] W_16^{q ka}         (ka < 16, i' < M)
+//   stage 2 (consumer)                 Z[ka + 16 k'] = sum_{i' < M} y[ka][i'] W_M^{i' k'}                     (k' < M)
 //
-// i.e. decimation in frequency with the first digit of radix K1.  Stage 1 only needs the K1 points {i' + 256 q} of a
-// row, so a CTA that runs the polyphase FIR (Eq. (1)) on the columns of 256 / K1 consecutive i' and
-// all q owns complete butterflies: its FIR warps put finished rows into a shared-memory tile, its butterfly warps
-// take them out again K1 at a time, and what goes to the next stage is y, laid out [antenna][spectrum][ka][i'].
-// Stage 2 is then K1 independent 256-point transforms per spectrum; ONE WARP does the two transforms ka and K1 - ka
-// (a channel k and its mirror n - k, which the real-FFT post-twiddle of PAPER.md:183 pairs, live in exactly these
-// two), 16 points x 2 pols per thread, with warp-level synchronisation only: radix 16, exchange through the warp's
-// own 8.5 KB of shared memory, radix 16, mirror exchange, then post-twiddle, fine-delay rotation,
-// gain and quantisation in registers.  The int8 words of a spectrum are collected in
-// a staging row per team of warps so that the global stores are full 128-byte lines (a transform ka holds the
-// channels k = ka mod K1, 4 bytes every 4 K1 bytes).
-//
-// Against the one-CTA-per-spectrum FFT (fe_fft2.cuh) this moves a third of the butterflies next to the FIR, whose
-// kernel was bound by its scratch writes, and removes every CTA-wide barrier from the transform: the warps of an
-// SM are in different phases (loading, butterflies, exchange, stores) instead of stalling together.
+// i.e. decimation in frequency with the first digit of radix 16.  Stage 1 only needs the 16 points {i' + M q} of a
+// row, so a CTA that runs the polyphase FIR (Eq. (1)) on the columns of 16 consecutive i' and all q
+// owns complete butterflies: its FIR warps put finished rows into a shared-memory tile, its butterfly warps take them
+// out again 16 at a time, and what goes to the next stage is y, laid out [antenna][spectrum][ka][i'].
+// Stage 2 is then 16 independent M-point transforms per spectrum, and the real-FFT post-twiddle of PAPER.md:183 couples
+// exactly the transforms ka and 16 - ka (a channel k and its mirror n - k):
+//   M = 256 (n = 4096)          ONE WARP does the pair, 16 points x 2 pols per thread, warp-level synchronisation
+//                               only: radix 16, exchange through the warp's own 8.5 KB of shared memory, radix 16, mirror
+//                               exchange, then post-twiddle, fine-delay rotation, gain and
+//                               quantisation in registers; the int8 words of a spectrum are collected
+//                               in a staging row per CTA so that the global stores are full 128-byte lines;
+//   M = 1024, 2048 (n >= 16384)  one CTA of two teams does the pair with the pol-packed M-point plan of fe_fft2.cuh
+//                               (split_pair_kernel, further down).
+// Measured: the default for n >= 16384 (config 3: 116 -> 158 Gsample/s); at n = 4096 the
+// consumer is faster than the one-CTA-per-spectrum FFT but the producer, with a third of the butterflies next to the
+// FIR, is FMA-issue bound, and the two-kernel path of fe_fir2.cuh / fe_fft2.cuh stays the default there.
 #pragma once
 #include "fe_common.cuh"
 #include "fe_fft.cuh"
