@@ -283,6 +283,7 @@ def test_other_sample_widths(torch, fb, bits, n, T, S, equal_pols):
     (1024, 16, 2, (-3000, 5000), [40, 17, 64], True),            # windows reach back and ahead of the chunk
     (4096, 8, 1, (-20000, 9000), [33, 90], False),               # unequal pols: one-pol kernels
     (64, 3, 2, (-200, 300), [5, 9, 2], False),                   # generic kernels
+    (16384, 16, 1, (-40000, 50000), [21, 40, 9], True),          # split path (default at n >= 16384)
 ])
 def test_streaming_pushes_equal_one_batch(torch, fb, n, T, A, crange, pushes, equal_pols):
     """fengine_stream_*: concatenated pushes == fengine_process on [D zero rows, stream]."""
@@ -614,11 +615,15 @@ def test_process_host_matches_device_path(torch, fb):
     (4096, 2, 131, (-9000, 20000), False, 5),        # windows reach back and forward over several rows
     (8192, 1, 70, (-20000, 3), True, 8),             # per-spectrum tables, non-packed kernels, reads ahead of the chunk
     (1024, 1, 40, (0, 5), False, 64),                # more chunks asked for than 4 per spectrum allows: plain path
+    (16384, 2, 50, (-30000, 70000), False, 4),       # split path (default at n >= 16384), equal pols below
 ])
 def test_process_host_pipeline_matches_device_path(torch, fb, n, A, S, crange, per_spectrum, chunks):
     """fengine_process_host cuts the call into pieces and overlaps H2D, kernels and D2H."""
     w = si.custom_workload(A=A, n=n, T=16, S=S, P=2, seed=41, per_spectrum=per_spectrum, coarse_range=crange)
+    if n >= 16384:
+        w.coarse[:, 1] = w.coarse[:, 0]
     fe = make_engine(fb, w, host_chunks=chunks)
+    assert fe.path() == ("split" if n >= 16384 else fe.path())
     dev = gpu_run(torch, fe, w, want=("int8",))["out"]
     pin_in = torch.from_numpy(w.packed.reshape(-1)).pin_memory()
     for _ in range(2):                               # staging buffers are reused by the second call
@@ -627,10 +632,12 @@ def test_process_host_pipeline_matches_device_path(torch, fb, n, A, S, crange, p
         np.testing.assert_array_equal(dev, pin_out.numpy())
 
 
-@pytest.mark.parametrize("n,A,P,S", [(1024, 2, 2, 300), (4096, 1, 2, 256), (1024, 1, 1, 70), (64, 2, 2, 513)])
+@pytest.mark.parametrize("n,A,P,S", [(1024, 2, 2, 300), (4096, 1, 2, 256), (1024, 1, 1, 70), (64, 2, 2, 513), (16384, 1, 2, 70)])
 def test_channel_major_heaps_are_the_transposed_records(torch, fb, n, A, P, S):
     """fengine_process_heaps: [A][heap][channel][256 spectra][pol][re,im], zero past S."""
     w = si.custom_workload(A=A, n=n, T=4 if n == 64 else 16, S=S, P=P, seed=43, random_weights=(n <= 64))
+    if n >= 16384:
+        w.coarse[:, 1] = w.coarse[:, 0]                          # equal pols: the split path
     fe = make_engine(fb, w)
     ref = oracle_run(w)["out"]                                   # [A][S][n][P][2], from the oracle
     n_heaps = (S + 255) // 256
