@@ -164,6 +164,41 @@ int fengine_stream_begin(fengine_t *fe, int64_t max_new_spectra, int64_t *delay_
 int fengine_stream_push(fengine_t *fe, const void *in_new, void *out, int64_t n_new, void *stream);
 int fengine_stream_end(fengine_t *fe);
 
+/*
+ * fengine_process_noalloc -- steps 1-7 in one call that allocates nothing, for callers that cannot
+ * call cudaMalloc: programs that gave the whole GPU to their own memory pool at start-up, real-time receive loops
+ * that cannot take the device-wide stall of an allocation, hosts that forbid allocation after
+ * initialisation.  There is no handle (creating one allocates): every table is a DEVICE pointer the caller owns, and
+ * the FIR -> transform intermediate lives in a fixed array built into the library (FENGINE_NOALLOC_MAX_FLOATS floats =
+ * 4 MiB of device memory, held by every GPU that loads the library until the process exits).
+ *
+ * in             DEVICE [A][P][L*5/4] bytes, 10-bit samples as fengine_process, L = N*(n_spectra + taps - 1), N = 2n.
+ * out            DEVICE [A][n_spectra][n][P][2] int8, as fengine_process.
+ * weights        DEVICE float [N*taps], weights[t + N*j] = w[t][j] of Eq. (1).
+ * coarse_delays  DEVICE int32 [A][P], one value per stream for the whole call.
+ * fine_delays, phases  DEVICE float [A][P].
+ * gains_re_im    DEVICE float [A][P][n][2], 8-byte aligned.
+ * n_channels     n, a power of two in [8, 32768]; taps 1..32; n_pols 1 or 2; n_antennas >= 1; n_spectra >= 0.
+ * stream         a cudaStream_t (NULL = default stream); kernels are enqueued, the call does not synchronise.
+ * err, err_len   HOST buffer for a message when the return value is not FENGINE_OK (may be NULL / 0).
+ *
+ * Limit: A * P * n_spectra * N <= FENGINE_NOALLOC_MAX_FLOATS (e.g. 128 spectra of one dual-pol antenna at n = 2048);
+ * a larger call is refused with FENGINE_ERR_INVALID_ARG and a message that states the limit -- split the batch.
+ * The caller's tables are read as they are at kernel run time and are not validated (non-finite values propagate).
+ * Runs the simple one-thread-per-output kernels (the "force_generic" path of fengine_process), so the result is that
+ * path's; it is not the fast path.
+ * First call on a device: looks up the device address of the built-in array (once per device; no allocation).  Make
+ * that first call with the device current and before any stream capture begins.
+ * All calls on a device share the array, which keeps the previous call's contents (every word that is read is written
+ * first by the same call, so nothing needs clearing).  Calls whose kernels may overlap on the GPU -- two streams with no
+ * event between them, two host threads -- race on it: serialise them.
+ */
+#define FENGINE_NOALLOC_MAX_FLOATS (1 << 20)
+int fengine_process_noalloc(const void *in, void *out, const float *weights, const int32_t *coarse_delays,
+                            const float *fine_delays, const float *phases, const float *gains_re_im,
+                            int n_antennas, int n_channels, int taps, int n_pols, int64_t n_spectra,
+                            void *stream, char *err, int64_t err_len);
+
 /* Human-readable description of the last error on this handle ("" if none). */
 const char *fengine_last_error(const fengine_t *fe);
 

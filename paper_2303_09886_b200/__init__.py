@@ -12,4 +12,6 @@ from .binding import (  # noqa: F401
     library_path,
     EXPORTED_SYMBOLS,
     fp32_rate,
+    process_noalloc,
+    NOALLOC_MAX_FLOATS,
 )

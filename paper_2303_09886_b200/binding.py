@@ -17,6 +17,7 @@ EXPORTED_SYMBOLS = [
     "fengine_last_error", "fengine_process_f32", "fengine_debug_unpack", "fengine_debug_fir",
     "fengine_set_option", "fengine_last_launch_count", "fengine_profile_read", "fengine_process_heaps",
     "fengine_stream_begin", "fengine_stream_push", "fengine_stream_end", "fengine_reserve", "fengine_debug_pipe_stats", "fengine_debug_fp32_rate", "fengine_debug_path",
+    "fengine_process_noalloc",
 ]
 
 STATUS = {0: "OK", 1: "INVALID_ARG", 2: "ALLOC", 3: "CUDA", 4: "STATE"}
@@ -70,6 +71,8 @@ def lib() -> C.CDLL:
         L.fengine_profile_read.argtypes = [vp, vp, vp, vp, vp]
         L.fengine_last_launch_count.argtypes = [vp]
         L.fengine_last_launch_count.restype = i64
+        L.fengine_process_noalloc.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, i64, vp,
+                                              C.c_char_p, i64]
         _lib = L
     return _lib
 
@@ -117,6 +120,35 @@ def fp32_rate() -> float:
     if rc != 0:
         raise FEngineError(rc, "fengine_debug_fp32_rate failed")
     return float(r.value)
+
+
+NOALLOC_MAX_FLOATS = 1 << 20     # FENGINE_NOALLOC_MAX_FLOATS of include/fengine.h
+
+
+def process_noalloc(inp, out, weights, coarse, fine_delay, phase, gains, n_antennas: int, n_channels: int, taps: int,
+                    n_pols: int, n_spectra: int, stream=None):
+    """fengine_process_noalloc: the whole path for callers that must not allocate device memory (a program that gave
+    the GPU's memory to its own pool, a real-time loop that cannot stall on cudaMalloc).  No handle: every table is a
+    CUDA tensor the caller already holds (weights float32 [N*T], coarse int32 [A][P], fine_delay / phase float32
+    [A][P], gains float32 [A][P][n][2] or complex64 [A][P][n]); the intermediate lives in a 4 MiB array inside the
+    library, which bounds A*P*n_spectra*N to NOALLOC_MAX_FLOATS and is shared by all calls (do not overlap them).
+    Asynchronous on `stream`; make the first call on a device outside stream capture."""
+    A, n, T, P, S = int(n_antennas), int(n_channels), int(taps), int(n_pols), int(n_spectra)
+    N = 2 * n
+    s_pos = max(S, 0)
+    args = [
+        _dev_buf(inp, A * P * (N * (s_pos + T - 1) * 10 // 8) if s_pos else 0, "input", ("uint8", "int8")),
+        _dev_buf(out, A * s_pos * n * P * 2, "output", ("int8", "uint8")),
+        _dev_buf(weights, N * T * 4, "weights", ("float32",)),
+        _dev_buf(coarse, A * P * 4, "coarse", ("int32",)),
+        _dev_buf(fine_delay, A * P * 4, "fine_delay", ("float32",)),
+        _dev_buf(phase, A * P * 4, "phase", ("float32",)),
+        _dev_buf(gains, A * P * n * 8, "gains", ("float32", "complex64")),
+    ]
+    err = C.create_string_buffer(512)
+    rc = lib().fengine_process_noalloc(*args, A, n, T, P, S, _stream_handle(stream), err, len(err))
+    if rc != 0:
+        raise FEngineError(rc, err.value.decode())
 
 
 class FEngine:
