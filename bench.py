@@ -42,6 +42,19 @@ def csrc_hash() -> str:
     return h.hexdigest()
 
 
+def workload_stamp(args, w=None) -> str:
+    """What was measured, as one string: the second stamp of profiles/roofline_traffic.csv (the ncu capture there is of
+    ONE workload and option set; a run of anything else must not report its DRAM bytes)."""
+    opts = sorted(args.opt)
+    if args.chunk_spectra is not None:
+        opts.append(f"chunk_spectra={args.chunk_spectra}")
+    if args.fir_rows is not None:
+        opts.append(f"fir_rows={args.fir_rows}")
+    shape = f"n={w.n};T={w.T};A={w.A};S={w.S}" if w is not None else \
+        f"n={args.n_channels or 'default'};T={args.taps or 'default'};S={args.n_spectra or 'default'}"
+    return f"config={args.config};{shape};bits={args.sample_bits};opts={'+'.join(opts)}"
+
+
 def measured_peaks():
     f = ROOT / "MEASURED_PEAKS.json"
     if f.exists():
@@ -308,14 +321,20 @@ def main():
     prof = ROOT / "profiles" / "roofline_traffic.csv"
     roofline["traffic_step"] = None
     if prof.exists():
-        rows, src_hash = {}, None
+        rows, src_hash, src_workload = {}, None, None
         for ln in prof.read_text().splitlines():
             if ln.startswith("# csrc_sha256="):
                 src_hash = ln.split("=", 1)[1].strip()
+            if ln.startswith("# workload="):
+                src_workload = ln.split("=", 1)[1].strip()
             parts = ln.split(",")
             if len(parts) == 2 and parts[1].isdigit():
                 rows[parts[0]] = int(parts[1])
-        if src_hash == csrc_hash():
+        roofline["traffic_workload"] = workload_stamp(args, w)
+        if src_workload != roofline["traffic_workload"]:
+            roofline["traffic_source"] = (f"withheld: the committed ncu capture is of another workload or option set "
+                                          f"({src_workload}; profiles/roofline_traffic.csv)")
+        elif src_hash == csrc_hash():
             roofline["traffic"] = rows.get(dom_name)
             names = ["fused_kernel"] if roofline["fused"] else ["fir_kernel", "fft_kernel"]
             if all(nm in rows for nm in names):

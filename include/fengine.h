@@ -209,11 +209,17 @@ int fengine_process_f32(fengine_t *fe, const void *in, float *spectra_out, int64
                         void *stream);
 
 /* Unpacked, coarse-delayed window samples: DEVICE int16 [A][P][n_spectra][N*T] (small cases only):
- * element i of spectrum m is s[N*m - c + i] (0 outside the batch).  Bit-exact check of steps 1-2. */
+ * element i of spectrum m is s[N*m - c + i] (0 outside the batch).  Bit-exact check of steps 1-2.
+ * This hook runs a one-thread-per-sample SIDE kernel that no timed configuration launches; the unpackers of the
+ * kernels fengine_process runs are checked bit-exactly through fengine_debug_fir with one-hot weights (fir_kernel,
+ * fir2_kernel, fir3_kernel) and, where the rows never leave the chip as integers (split producer, pipelined kernel),
+ * through fengine_process_f32 with one-hot weights (tests/test_gpu_parity.py). */
 int fengine_debug_unpack(fengine_t *fe, const void *in, int16_t *samples_out, int64_t n_spectra,
                          void *stream);
 
-/* FIR output g of Eq. (1) in natural column order: DEVICE float [A][P][n_spectra][N]. */
+/* FIR output g of Eq. (1) in natural column order: DEVICE float [A][P][n_spectra][N].  Runs the FIR kernel of the path
+ * fengine_debug_path reports for pol_packed, packed_fir_one_pol_fft, one_pol and generic; on the split and fused paths,
+ * whose FIR has no separate output, it runs the one-pol FIR kernel instead. */
 int fengine_debug_fir(fengine_t *fe, const void *in, float *g_out, int64_t n_spectra, void *stream);
 
 /* Tuning knobs (optional; defaults are chosen at create).  key: "chunk_spectra" (spectra per

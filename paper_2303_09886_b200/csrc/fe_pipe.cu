@@ -1,5 +1,7 @@
 // fe_pipe.cu -- instantiations and launcher of the pipelined kernel (fe_pipe.cuh); a translation unit of its own so
 // that it compiles in parallel with fengine.cu.
+#include <mutex>
+
 #include "fe_pipe.cuh"
 #include "fe_plans.cuh"
 
@@ -7,17 +9,35 @@ namespace fe {
 
 namespace {
 
+// The dynamic shared-memory limit is an attribute of the FUNCTION (per device), not of a handle: it is raised here,
+// never lowered, and remembered per instantiation and device, so that a second handle with fewer FIR warps cannot
+// shrink it under the first.  The CTAs of the kernel spin-wait on one another (FIR warps of one CTA feed the FFT team of
+// another), which is deadlock-free only when the whole grid is resident: the launch is a cooperative one, which the
+// runtime refuses (cudaErrorCooperativeLaunchTooLarge) unless every CTA fits on the device at once and which is not
+// started piecemeal beside kernels of other streams or handles.
 template <int T, class Plan, bool F32OUT>
-cudaError_t launch_one(const PipeParams &prm, int grid, bool set_attr, cudaStream_t stream)
+cudaError_t launch_one(const PipeParams &prm, int grid, bool /*set_attr*/, cudaStream_t stream)
 {
+    static std::mutex mu;
+    static size_t limit_set[64] = {};
     const size_t smem = PipeSmem<Plan>::bytes(prm.fir_warps);
-    if (set_attr) {
-        cudaError_t e = cudaFuncSetAttribute(pipe_kernel<T, Plan, F32OUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    {
+        std::lock_guard<std::mutex> lock(mu);
+        if (smem > limit_set[dev]) {
+            e = cudaFuncSetAttribute(pipe_kernel<T, Plan, F32OUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+            limit_set[dev] = smem;
+        }
     }
     const int threads = Plan::tpf + 64 + 32 * prm.fir_warps;      // team + loader + flow + FIR warps
-    pipe_kernel<T, Plan, F32OUT><<<grid, threads, smem, stream>>>(prm);
-    return cudaGetLastError();
+    PipeParams arg = prm;
+    void *args[] = {&arg};
+    return cudaLaunchCooperativeKernel(reinterpret_cast<const void *>(&pipe_kernel<T, Plan, F32OUT>), dim3((unsigned)grid),
+                                       dim3((unsigned)threads), args, smem, stream);
 }
 
 template <int T, bool F32OUT>

@@ -513,6 +513,33 @@ GenParams gen_params(const fengine *fe, const void *in, int64_t S)
 
 unsigned gen_grid(const fengine *fe, int64_t total) { return (unsigned)std::min<int64_t>((total + 255) / 256, (int64_t)fe->n_sms * 16); }
 
+// What a call over `Sr` spectra needs besides its inputs and outputs: ONE rule, used by process_impl (which sizes the
+// buffers on demand) and by fengine_reserve (which sizes them ahead), so that a reserve for S spectra always covers a
+// call of S spectra on the path the handle would take now.
+struct CallNeed {
+    bool fused;             // the pipelined kernel: an L2 ring and counters (ensure_pipe), no full-size scratch
+    bool split;             // fe_split.cuh
+    int64_t chunk;          // spectra per scratch-resident chunk
+    size_t scratch_floats;  // FP32 words of FIR -> FFT scratch (0 when fused)
+};
+CallNeed call_need(const fengine *fe, int64_t Sr)
+{
+    CallNeed c{};
+    const size_t streams = (size_t)fe->A * fe->P;
+    if (!use_tiled(fe)) {                                   // generic kernels: the whole call at once, chunk_spectra ignored
+        c.chunk = Sr;
+        c.scratch_floats = streams * (size_t)Sr * fe->N;
+        return c;
+    }
+    c.chunk = fe->chunk_spectra > 0 ? std::min<int64_t>(fe->chunk_spectra, Sr) : Sr;
+    c.fused = use_fused(fe) && !fe->scratch_h16;
+    c.split = !c.fused && use_split(fe) && !fe->scratch_h16;
+    // the n >= 16384 split consumer has the chunk's spectra in gridDim.y (limit 65535): longer calls run in chunks
+    if (c.split && split_is_big(fe->n)) c.chunk = std::min<int64_t>(c.chunk, 65535);
+    c.scratch_floats = c.fused ? 0 : streams * (size_t)c.chunk * fe->N;
+    return c;
+}
+
 // every entry point runs on the device the handle was created on
 int check_device(fengine *fe)
 {
@@ -579,7 +606,7 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
     const int streams = fe->A * fe->P;
 
     if (!use_tiled(fe)) {
-        int rc = ensure_scratch(fe, (size_t)streams * S * fe->N);
+        int rc = ensure_scratch(fe, call_need(fe, S).scratch_floats);
         if (rc) return rc;
         const GenParams gp = gen_params(fe, in, S);
         gen_fir_kernel<<<gen_grid(fe, (int64_t)streams * S * fe->N), 256, 0, stream>>>(gp, fe->d_scratch);
@@ -595,13 +622,13 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
     const bool per_spectrum = fe->n_coarse != 1 || fe->n_fine != 1;
     if (fe->rg_dirty) return fail(fe, FENGINE_ERR_STATE, "rotation / gain tables are stale (a setter failed)");
 
-    const int64_t chunk = fe->chunk_spectra > 0 ? std::min<int64_t>(fe->chunk_spectra, m_hi - m_lo) : m_hi - m_lo;
-    const bool fused = use_fused(fe) && !fe->scratch_h16;
-    const bool split = !fused && use_split(fe) && !fe->scratch_h16;
+    const CallNeed need = call_need(fe, m_hi - m_lo);
+    const int64_t chunk = need.chunk;
+    const bool fused = need.fused, split = need.split;
     if (fe->scratch_h16 && !(use_packed(fe) && fe->bits == 10))
         return fail(fe, FENGINE_ERR_STATE, "scratch_fp16 needs the pol-packed path (equal coarse delays in both pols, 10-bit samples)");
 
-    int rc = fused ? FENGINE_OK : ensure_scratch(fe, (size_t)streams * chunk * fe->N);
+    int rc = fused ? FENGINE_OK : ensure_scratch(fe, need.scratch_floats);
     if (rc) return rc;
     if (fe->l2_persist) {
         int max_win = 0;
@@ -785,6 +812,8 @@ int process_impl(fengine *fe, const void *in, int8_t *out, float *out_f32, int64
         if (fe->profile) FE_CUDA(fe, cudaEventRecord(ev[1], stream));
         if (packed && fe->allow_fft2p && fft2p_supported(fe->n) && !fe->scratch_h16) {
             bool &attr = fe->fft2p_attr[out_f32 ? 1 : 0];
+            if ((m1 - m0) * (int64_t)fe->A >= ((int64_t)1 << 31))   // the kernel counts (spectrum, antenna) rows in an int
+                return fail(fe, FENGINE_ERR_INVALID_ARG, "fft_persistent: more than 2^31 rows in a chunk; set chunk_spectra");
             const int grid = (int)std::min<int64_t>(fe->n_sms, (m1 - m0) * fe->A);
             cudaError_t ce = fft2p_launch(fe->n, out_f32 != nullptr, xp2, fe->A, grid, !attr, stream);
             attr = true;
@@ -956,6 +985,7 @@ int fengine_set_coarse_delays(fengine_t *fe, const int32_t *c, int64_t n_per_str
 try {
     if (!fe) return FENGINE_ERR_INVALID_ARG;
     fe->err.clear();
+    if (int rc = check_device(fe)) return rc;          // the handle's tables live on its own device
     if (!c || n_per_stream < 1) return fail(fe, FENGINE_ERR_INVALID_ARG, "bad coarse delay table");
     const size_t count = (size_t)fe->A * fe->P * n_per_stream;
     FE_CUDA(fe, cudaDeviceSynchronize());
@@ -999,6 +1029,7 @@ int fengine_set_fine_delays(fengine_t *fe, const float *delay, const float *phas
 try {
     if (!fe) return FENGINE_ERR_INVALID_ARG;
     fe->err.clear();
+    if (int rc = check_device(fe)) return rc;          // the handle's tables live on its own device
     if (!delay || !phase || n_per_stream < 1) return fail(fe, FENGINE_ERR_INVALID_ARG, "bad fine delay table");
     const size_t count = (size_t)fe->A * fe->P * n_per_stream;
     if (!all_finite(delay, count) || !all_finite(phase, count))
@@ -1031,6 +1062,7 @@ int fengine_set_gains(fengine_t *fe, const float *gains_re_im)
 try {
     if (!fe) return FENGINE_ERR_INVALID_ARG;
     fe->err.clear();
+    if (int rc = check_device(fe)) return rc;          // the handle's tables live on its own device
     if (!gains_re_im) return fail(fe, FENGINE_ERR_INVALID_ARG, "null gains");
     const size_t count = (size_t)fe->A * fe->P * fe->n;
     if (!all_finite(gains_re_im, count * 2)) return fail(fe, FENGINE_ERR_INVALID_ARG, "non-finite gain");
@@ -1060,15 +1092,16 @@ int fengine_reserve(fengine_t *fe, int64_t max_spectra)
 try {
     if (!fe) return FENGINE_ERR_INVALID_ARG;
     fe->err.clear();
+    if (int rc = check_device(fe)) return rc;          // the handle's tables live on its own device
     if (max_spectra < 1) return fail(fe, FENGINE_ERR_INVALID_ARG, "max_spectra < 1");
     fe->reserved = false;                                   // this call may allocate; later process calls may not
+    const CallNeed need = call_need(fe, max_spectra);       // the rule process_impl applies to a call of max_spectra
     int rc = FENGINE_OK;
-    if (use_tiled(fe) && use_fused(fe)) {
+    if (need.fused) {
         // the ring does not depend on S; the counters grow with it (every smaller call needs no more of either)
         rc = ensure_pipe(fe, pipe_plan(fe, max_spectra));
     } else {
-        const int64_t chunk = fe->chunk_spectra > 0 ? std::min<int64_t>(fe->chunk_spectra, max_spectra) : max_spectra;
-        rc = ensure_scratch(fe, (size_t)fe->A * fe->P * (size_t)chunk * fe->N);
+        rc = ensure_scratch(fe, need.scratch_floats);
     }
     if (rc) return rc;
     FE_CUDA(fe, cudaDeviceSynchronize());
@@ -1143,6 +1176,7 @@ int fengine_stream_begin(fengine_t *fe, int64_t max_new_spectra, int64_t *delay_
 try {
     if (!fe) return FENGINE_ERR_INVALID_ARG;
     fe->err.clear();
+    if (int rc = check_device(fe)) return rc;          // the handle's tables live on its own device
     if (max_new_spectra < 1) return fail(fe, FENGINE_ERR_INVALID_ARG, "max_new_spectra < 1");
     FE_CUDA(fe, cudaDeviceSynchronize());
     const int64_t back = ceil_div_rows(fe->c_max, fe->lgN) + 1;       // rows a positive delay (and a lagging column) reach back
@@ -1213,6 +1247,7 @@ int fengine_stream_end(fengine_t *fe)
 try {
     if (!fe) return FENGINE_ERR_INVALID_ARG;
     fe->err.clear();
+    if (int rc = check_device(fe)) return rc;          // the handle's tables live on its own device
     FE_CUDA(fe, cudaDeviceSynchronize());
     fe->stream_off = 0;
     return upload_coarse(fe);
@@ -1226,6 +1261,7 @@ int fengine_process_host(fengine_t *fe, const void *in_host, void *out_host, int
 try {
     if (!fe) return FENGINE_ERR_INVALID_ARG;
     fe->err.clear();
+    if (int rc = check_device(fe)) return rc;          // the handle's tables live on its own device
     if (n_spectra < 0) return fail(fe, FENGINE_ERR_INVALID_ARG, "n_spectra < 0");
     if (n_spectra == 0) return FENGINE_OK;
     if (!in_host || !out_host) return fail(fe, FENGINE_ERR_INVALID_ARG, "null host pointer");
@@ -1412,6 +1448,7 @@ int fengine_set_option(fengine_t *fe, const char *key, int64_t value)
 try {
     if (!fe || !key) return FENGINE_ERR_INVALID_ARG;
     fe->err.clear();
+    if (int rc = check_device(fe)) return rc;          // the handle's tables live on its own device
     if (fe->stream_off != 0 && (!strcmp(key, "sample_bits") || !strcmp(key, "force_generic") || !strcmp(key, "pol_packed") ||
                                 !strcmp(key, "fused") || !strcmp(key, "split") || !strcmp(key, "scratch_fp16")))
         return fail(fe, FENGINE_ERR_STATE, "option %s changes the data layout or the path and cannot change while a stream is open", key);
@@ -1506,6 +1543,7 @@ int fengine_profile_read(fengine_t *fe, double *fir_ms, double *fft_ms, int64_t 
 try {
     if (!fe) return FENGINE_ERR_INVALID_ARG;
     fe->err.clear();
+    if (int rc = check_device(fe)) return rc;          // the handle's tables live on its own device
     double fir = 0.0, fft = 0.0;
     int64_t count = 0;
     for (size_t i = 0; i + 2 < fe->ev_used.size(); i += 3) {
@@ -1536,6 +1574,7 @@ int fengine_debug_pipe_stats(fengine_t *fe, uint64_t *out, int64_t max_words)
 {
     if (!fe || !out) return FENGINE_ERR_INVALID_ARG;
     fe->err.clear();
+    if (int rc = check_device(fe)) return rc;          // the handle's tables live on its own device
     if (!fe->d_stats) return fail(fe, FENGINE_ERR_STATE, "option pipe_stats is off");
     const int64_t words = std::min<int64_t>(max_words, (int64_t)kStCount * fe->n_sms);
     FE_CUDA(fe, cudaDeviceSynchronize());

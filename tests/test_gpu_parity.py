@@ -119,29 +119,96 @@ def test_unpack_and_coarse_delay_bit_exact(torch, fb, case):
     np.testing.assert_array_equal(d_s.cpu().numpy(), _oracle_windows(w))
 
 
-@pytest.mark.parametrize("n,T,c", [(1024, 16, 0), (1024, 16, 3), (4096, 16, 4093), (4096, 8, -5), (2048, 4, 70001),
-                                    (8192, 16, 16382), (1024, 2, 2047), (4096, 32, 777), (1024, 32, -3000)])
-def test_tiled_fir_unpack_is_bit_exact_with_one_hot_weights(torch, fb, n, T, c):
-    """weights = 1 at one tap: the tiled FIR must return the delayed integer samples exactly."""
+def _delay_table(kind, c, S):
+    """int32 [1][2][1 or S]: 'equal' = both pols c; 'unequal' = (c, c + 5); 'steps' = both pols c + m // 8 (a new delay
+    every 8 spectra, BASELINE.json configs[3]); 'unequal_steps' = pol 1 runs 3 samples and one step pattern apart."""
+    m = np.arange(S)
+    if kind == "equal":
+        tab = np.full((1, 2, 1), c)
+    elif kind == "unequal":
+        tab = np.array([c, c + 5]).reshape(1, 2, 1)
+    elif kind == "steps":
+        tab = np.broadcast_to(c + m // 8, (1, 2, S))
+    else:
+        tab = np.stack([c + m // 8, c + 3 + m // 5]).reshape(1, 2, S)
+    return np.ascontiguousarray(tab, dtype=np.int32)
+
+
+@pytest.mark.parametrize("n,T,c,kind,path", [
+    (1024, 16, 0, "equal", "pol_packed"), (1024, 16, 3, "equal", "pol_packed"), (4096, 16, 4093, "equal", "pol_packed"),
+    (4096, 8, -5, "equal", "pol_packed"), (2048, 4, 70001, "equal", "pol_packed"), (8192, 16, 16382, "equal", "pol_packed"),
+    (1024, 2, 2047, "equal", "pol_packed"), (4096, 32, 777, "equal", "pol_packed"), (1024, 32, -3000, "equal", "pol_packed"),
+    (4096, 16, 8190, "steps", "pol_packed"), (2048, 32, -9, "steps", "pol_packed"),
+    (1024, 16, 3, "unequal", "one_pol"), (4096, 16, -4097, "unequal", "one_pol"), (4096, 8, 20000, "unequal", "one_pol"),
+    (1024, 16, 2040, "unequal_steps", "one_pol"), (8192, 4, 16380, "unequal_steps", "one_pol"),
+    (16384, 16, 77, "unequal", "one_pol"),
+])
+def test_tiled_fir_unpack_is_bit_exact_with_one_hot_weights(torch, fb, n, T, c, kind, path):
+    """weights = 1 at one tap: the FIR kernel fengine_process launches for this shape (fir2_kernel / fir3_kernel when the
+    two pols share their delays, fir_kernel when they do not) must return the integer rows the float64 side gets from
+    oracle.unpack10 + oracle.window, exactly (steps 1-2): every row of the batch, the last one
+    included, for c < 0, c > N and per-spectrum delay steps."""
     N = 2 * n
     S = 70
-    w = si.custom_workload(A=1, n=n, T=T, S=S, seed=23)
+    w = si.custom_workload(A=1, n=n, T=T, S=S, seed=23, keep_samples=False)
     j0 = T // 2
     h = np.zeros(N * T, dtype=np.float32)
     h[N * j0:N * (j0 + 1)] = 1.0
     fe = fb.FEngine(n, T, 2, h, n_antennas=1)
-    fe.set_coarse_delays(np.full((1, 2, 1), c, np.int32))
+    tab = _delay_table(kind, c, S)
+    fe.set_coarse_delays(tab)
+    assert fe.path() == path
     d_in = torch.from_numpy(w.packed.reshape(-1)).cuda()
-    d_g = torch.zeros((1, 2, S, N), dtype=torch.float32, device="cuda")
+    d_g = torch.full((1, 2, S, N), float("nan"), dtype=torch.float32, device="cuda")
     fe.debug_fir(d_in, d_g, S)
     torch.cuda.synchronize()
     g = d_g.cpu().numpy()
     for p in range(2):
-        s = w.samples[0, p].astype(np.int64)
-        idx = N * np.arange(S)[:, None] - c + N * j0 + np.arange(N)[None, :]
-        ok = (idx >= 0) & (idx < s.size)
-        expect = np.where(ok, s[np.clip(idx, 0, s.size - 1)], 0)
-        np.testing.assert_array_equal(g[0, p], expect.astype(np.float32))
+        s = oracle.unpack10(w.packed[0, p], w.L).astype(np.float64)
+        for m in range(S):
+            cm = int(tab[0, p, m if tab.shape[2] > 1 else 0])
+            expect = oracle.window(s, N, T, m, cm)[N * j0:N * (j0 + 1)]
+            np.testing.assert_array_equal(g[0, p, m], expect.astype(np.float32), err_msg=f"pol {p} spectrum {m}")
+
+
+@pytest.mark.parametrize("n,T,c,kind,opts,path", [
+    (4096, 16, 4093, "equal", {"split": 1}, "split"), (4096, 8, -4100, "steps", {"split": 1}, "split"),
+    (16384, 16, 32767, "equal", {}, "split"), (16384, 4, -40000, "steps", {}, "split"),
+    (32768, 16, 65531, "steps", {}, "split"), (32768, 8, -3, "equal", {}, "split"),
+    (1024, 16, 2047, "equal", {"fused": 1}, "fused"), (4096, 16, -5, "steps", {"fused": 1}, "fused"),
+    (4096, 16, 9000, "steps", {}, "pol_packed"), (4096, 16, 9000, "unequal_steps", {}, "one_pol"),
+    (32768, 32, 100, "equal", {}, "packed_fir_one_pol_fft"),
+])
+def test_unpack_and_delay_are_exact_through_the_kernels_of_every_path(torch, fb, n, T, c, kind, opts, path):
+    """Steps 1-2 through kernels that have no integer output to look at (the split producer
+    runs the first radix-16 stage on its rows before they leave shared memory, the pipelined kernel hands rows to the
+    transform through its ring): with weights = 1 at one tap, unit gain and no fine delay the spectrum of the float64
+    side is the plain transform of the integer row oracle.unpack10 + oracle.window select.  One wrong sample, off by
+    e >= 1 LSB, moves EVERY channel of that spectrum by e in modulus (>= 0.707 e in its larger component); any error
+    pattern other than a pure (-1)^t alternation moves some kept channel by >= 0.5.  The FP32 rounding error of the
+    transform is 2e-5 x RMS at most (sigma = 8 keeps the RMS below 4000 at N = 65536, i.e. < 0.08), so a bound of 0.3
+    on every real and imaginary part separates "every sample exact" from "some sample wrong"."""
+    N = 2 * n
+    S = 70
+    w = si.custom_workload(A=1, n=n, T=T, S=S, seed=29, sigma=8.0, keep_samples=False)
+    j0 = T - 1 if T < 4 else T // 2 + 1
+    h = np.zeros(N * T, dtype=np.float32)
+    h[N * j0:N * (j0 + 1)] = 1.0
+    tab = _delay_table(kind, c, S)
+    fe = fb.FEngine(n, T, 2, h, n_antennas=1)
+    fe.set_coarse_delays(tab)
+    for k, v in opts.items():
+        fe.set_option(k, v)
+    assert fe.path() == path
+    d_in = torch.from_numpy(w.packed.reshape(-1)).cuda()
+    d_y = torch.full(fe.output_shape(S), float("nan"), dtype=torch.float32, device="cuda")
+    fe.process_f32(d_in, d_y, S)
+    torch.cuda.synchronize()
+    y = d_y.cpu().numpy().astype(np.float64)
+    ref = oracle.process(w.packed, 1, n, T, 2, h, S, coarse=tab)["Y"]
+    err = np.maximum(np.abs(y[..., 0] - ref.real), np.abs(y[..., 1] - ref.imag))
+    assert np.sqrt(np.mean(np.abs(ref) ** 2)) > 100.0                   # the rows are not trivially zero
+    assert err.max() < 0.3, f"{path}: a channel is off by {err.max():.3f} LSB: some sample of the row is wrong"
 
 
 # ----------------------------------------------------------------------------------------------
@@ -743,6 +810,53 @@ def test_reserve_makes_process_allocation_free_and_capturable(torch, fb, cfg, op
     g.replay()
     torch.cuda.synchronize()
     check_parity({"out": d_out.cpu().numpy()}, ref, "graph replay")
+
+
+@pytest.mark.parametrize("shape,opts", [
+    (dict(A=1, n=64, T=3, S=24), {"chunk_spectra": 5}),                  # generic kernels ignore chunk_spectra
+    (dict(A=1, n=1024, T=16, S=40), {"fused": 1, "scratch_fp16": 1}),   # FP16 scratch wins over the pipelined kernel
+    (dict(A=2, n=1024, T=16, S=40), {"chunk_spectra": 16}),
+])
+def test_reserve_covers_the_call_it_was_made_for(torch, fb, shape, opts):
+    """fengine_reserve(S) and fengine_process size their buffers by one rule: after a successful reserve a call of S
+    spectra never fails with FENGINE_ERR_STATE, whatever path and chunking the options select."""
+    w = si.custom_workload(coarse_range=(0, 1), **shape, keep_samples=False)
+    fe = make_engine(fb, w, **opts)
+    fe.reserve(w.S)
+    d_in = torch.from_numpy(w.packed.reshape(-1)).cuda()
+    d_out = torch.full(fe.output_shape(w.S), 99, dtype=torch.int8, device="cuda")
+    fe.process(d_in, d_out, w.S)
+    torch.cuda.synchronize()
+    assert bool((d_out != 99).any())
+    if "scratch_fp16" not in opts:
+        check_parity({"out": d_out.cpu().numpy()}, oracle_run(w), f"reserved {opts}")
+
+
+def test_calls_made_on_another_device_are_refused(torch, fb):
+    """include/fengine.h: a handle belongs to the device that was current at create; EVERY entry point that touches CUDA
+    (setters, reserve, streaming, options, the host path) refuses a call made with another device current, before it
+    allocates or launches anything there."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two CUDA devices")
+    w = si.make_workload(1, n_spectra=8)
+    torch.cuda.set_device(0)
+    fe = make_engine(fb, w)
+    host_out = np.zeros(fe.output_shape(w.S), np.int8)
+    try:
+        torch.cuda.set_device(1)
+        free1 = torch.cuda.mem_get_info(1)[0]
+        for call in (lambda: fe.set_coarse_delays(w.coarse), lambda: fe.set_fine_delays(w.fine_delay, w.phase),
+                     lambda: fe.set_gains(w.gains), lambda: fe.reserve(w.S), lambda: fe.stream_begin(4),
+                     lambda: fe.stream_end(), lambda: fe.set_option("chunk_spectra", 4),
+                     lambda: fe.process_host(w.packed.reshape(-1), host_out, w.S)):
+            with pytest.raises(fb.FEngineError) as e:
+                call()
+            assert e.value.code == 4
+        assert torch.cuda.mem_get_info(1)[0] == free1                 # nothing was allocated on the wrong device
+    finally:
+        torch.cuda.set_device(0)
+    got = gpu_run(torch, fe, w)                                        # and the handle still works on its own device
+    check_parity(got, oracle_run(w), "after refused calls")
 
 
 def test_setters_take_effect_between_calls(torch, fb):

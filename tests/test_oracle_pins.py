@@ -407,3 +407,28 @@ def test_unpack_bits_at_10_bits_is_unpack10_and_hand_examples():
     np.testing.assert_array_equal(oracle.unpack_bits(np.array([0x1F, 0x78], np.uint8), 4, 4), [1, -1, 7, -8])
     np.testing.assert_array_equal(oracle.unpack_bits(np.array([0x00, 0x1F, 0xFF], np.uint8), 2, 12), [1, -1])
     np.testing.assert_array_equal(oracle.unpack_bits(np.array([0xFF, 0xFE], np.uint8), 1, 16), [-2])
+
+
+def test_one_lsb_in_one_sample_moves_every_channel_of_a_one_hot_spectrum():
+    """The detection bound used by tests/test_gpu_parity.py::test_unpack_and_delay_are_exact_through_the_kernels_of_every_path:
+    with weights = 1 at one tap, unit gain and no fine delay the spectrum is the transform of one integer row
+    (PAPER.md:33-37), so one sample that is off by 1 LSB changes every channel by exactly 1 in modulus, i.e. by at least
+    0.707 in its larger component -- far above that test's 0.3 bound."""
+    n, T, S = 64, 4, 5
+    N = 2 * n
+    w = si.custom_workload(A=1, n=n, T=T, S=S, seed=3, sigma=8.0)
+    j0 = 3
+    h = np.zeros(N * T, dtype=np.float32)
+    h[N * j0:N * (j0 + 1)] = 1.0
+    c = np.array([[[5], [-9]]], dtype=np.int32)
+    base = oracle.process(w.packed, 1, n, T, 2, h, S, coarse=c)["Y"]
+    s = w.samples.copy()
+    m, t = 2, 37
+    u = N * (m + j0) - int(c[0, 1, 0]) + t                    # the sample row j0 of spectrum m reads at column t (pol 1)
+    s[0, 1, u] += 1 if s[0, 1, u] < 511 else -1
+    moved = oracle.process(si.pack10(s), 1, n, T, 2, h, S, coarse=c)["Y"]
+    d = moved - base
+    np.testing.assert_allclose(np.abs(d[0, m, :, 1]), 1.0, atol=1e-9)
+    assert np.maximum(np.abs(d.real), np.abs(d.imag))[0, m, :, 1].min() >= 0.7
+    d[0, m, :, 1] = 0
+    assert np.abs(d).max() < 1e-9                             # and nothing else moves
