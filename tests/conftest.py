@@ -11,6 +11,7 @@ if str(ROOT) not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (B200); run with -m gpu")
+    config.addinivalue_line("markers", "slow: a GPU test that runs for tens of seconds (deselect with -m 'gpu and not slow')")
 
 
 def pytest_collection_modifyitems(config, items):
