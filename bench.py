@@ -50,6 +50,8 @@ def workload_stamp(args, w=None) -> str:
         opts.append(f"chunk_spectra={args.chunk_spectra}")
     if args.fir_rows is not None:
         opts.append(f"fir_rows={args.fir_rows}")
+    if getattr(args, "pol_offset", 0):
+        opts.append(f"pol_offset={args.pol_offset}")
     shape = f"n={w.n};T={w.T};A={w.A};S={w.S}" if w is not None else \
         f"n={args.n_channels or 'default'};T={args.taps or 'default'};S={args.n_spectra or 'default'}"
     return f"config={args.config};{shape};bits={args.sample_bits};opts={'+'.join(opts)}"
@@ -170,6 +172,9 @@ def main():
     ap.add_argument("--n-spectra", type=int, default=None, help="shrink the batch (debugging only)")
     ap.add_argument("--sample-bits", type=int, default=10, help="input sample width (bit-depth sweep of PAPER.md:273-279)")
     ap.add_argument("--taps", type=int, default=None, help="override T (tap sweep of PAPER.md:235-249; 2, 4, 8, 16, 32)")
+    ap.add_argument("--pol-offset", type=int, default=0,
+                    help="add this many samples to the coarse delay of pol 1 of every antenna (PAPER.md:117: the two "
+                         "polarisations may have different delays): measures the kernels an unequal-pol engine runs")
     ap.add_argument("--chunk-spectra", type=int, default=None)
     ap.add_argument("--fir-rows", type=int, default=None)
     ap.add_argument("--opt", action="append", default=[], help="library option key=value (fengine_set_option), repeatable")
@@ -202,6 +207,9 @@ def main():
     # (weak scaling, no data-path collective).  Different seed per rank = different antennas.
     w = si.make_workload(args.config, n_spectra=args.n_spectra, n_channels=args.n_channels, seed=rank, taps=args.taps, bits=args.sample_bits)
     fe = fb.FEngine(w.n, w.T, w.P, w.weights, n_antennas=w.A)
+    if args.pol_offset:
+        w.coarse = w.coarse.copy()
+        w.coarse[:, 1] += args.pol_offset
     fe.set_coarse_delays(w.coarse)
     fe.set_fine_delays(w.fine_delay, w.phase)
     fe.set_gains(w.gains)
@@ -382,7 +390,9 @@ def main():
             "ms_per_step": ms_per_step, "ms_per_step_stats": step_stats, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": f"config{args.config}: {w.A} antennas x {w.P} pols per GPU, n={w.n}, T={w.T}, "
-                                   f"{w.L} samples per pol per step, S={w.S} spectra",
+                                   f"{w.L} samples per pol per step, S={w.S} spectra"
+                                   + (f", pol 1 delayed by {args.pol_offset} more samples" if args.pol_offset else ""),
+                       "path": fe.path(),
                        "l2_hygiene": f"inputs larger than L2: {n_sets} rotating buffer sets, "
                                      f"{(in_bytes + out_bytes) / 1e6:.0f} MB touched per step",
                        "parallelism": f"antennas sharded over {world} GPU(s), no collective"},
