@@ -70,7 +70,7 @@ struct fengine {
     float4 *d_rg2s = nullptr;                            // d_rg2 in split order (fe_split.cuh: split_gidx)
     float2 *d_sp_ptw1 = nullptr, *d_sp_ptw2 = nullptr;   // n >= 16384: pass twiddles of the n/16-point plan of the pair kernel
     bool split_attr[3] = {};        // shared-memory attribute set (producer, consumer int8, consumer f32)
-    int ring_rows = 32;             // option "ring_rows" (D: rows per track, a power of two >= 16)
+    int ring_rows = 64;             // option "ring_rows" (D: rows per track, a power of two >= 16); 64 measured best (0.55 ms at config 2; 32: 0.71)
     int opt_fir_warps = 0;          // option "fir_warps" (FIR warps per CTA, 0 = as many as the block allows)
     int opt_tracks = 0;             // option "tracks" (J, 0 = as many as the FIR warps serve)
     int opt_segments = 0;           // option "segments" (K per antenna, 0 = chosen per call)
